@@ -1,0 +1,26 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+
+
+@pytest.fixture(scope="session")
+def workloads_cache():
+    """Seeded workloads are deterministic; build each once per session."""
+    from workloads import make_workload
+    cache = {}
+
+    def get(name, n_proj=None):
+        key = (name, n_proj)
+        if key not in cache:
+            cache[key] = make_workload(name, n_proj=n_proj)
+        return cache[key]
+    return get

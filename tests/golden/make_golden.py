@@ -1,0 +1,42 @@
+"""Writes tests/golden/oracle_regression.txt.  Calls ONLY oracle/ (and the input
+generator); never the CUDA path.
+
+The paper (arXiv 1204.6367) prints no numeric value of P(u) or of a line
+integral, so there is no paper-printed fixture to store.  This file freezes a
+few oracle outputs on C0 and C1 so that an accidental change to the oracle's
+arithmetic is noticed; it is a regression guard, not an independent pin (the
+independent pins are in tests/test_oracle_pins.py).
+
+    python tests/golden/make_golden.py
+"""
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+
+import oracle  # noqa: E402
+from workloads import make_workload  # noqa: E402
+
+PIXELS = {"C0": [(32, 24), (20, 17), (40, 30), (0, 0), (31, 9)],
+          "C1": [(128, 96), (10, 10), (200, 150), (77, 33), (255, 191)]}
+
+
+def main():
+    lines = ["# workload p i j j0 n signal LI_0 [LI_1 ...]   (oracle/gdrr_oracle.c, fp64)"]
+    for name, pix in PIXELS.items():
+        w = make_workload(name)
+        arr = np.array([[0, i, j] for i, j in pix])
+        out = oracle.project(w, pixels=arr)
+        for q, (i, j) in enumerate(pix):
+            li = " ".join(f"{x:.17g}" for x in out["line_integrals"][q])
+            lines.append(f"{name} 0 {i} {j} {out['ray_table'][q, 0]} {out['ray_table'][q, 1]} "
+                         f"{out['signal'][q]:.17g} {li}")
+    with open(os.path.join(os.path.dirname(__file__), "oracle_regression.txt"), "w") as f:
+        f.write("\n".join(lines) + "\n")
+
+
+if __name__ == "__main__":
+    main()
