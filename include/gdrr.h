@@ -1,0 +1,200 @@
+/*
+ * gdrr.h -- C ABI of the B200-native poly-energetic primary-signal projector
+ * of gDRR (Jia et al., arXiv 1204.6367, section 2.3).
+ *
+ * What it computes (Eq. (1) at PAPER.md:147):
+ *
+ *     P(u) = sum_E  phi_E * w(u) * exp(-mu_bt(E) t_bt(u)) * R_E
+ *                   * exp( - sum_m mu_hat_m(E) * LI_m(u) )
+ *     LI_m(u) = dl * sum_k  trilinear(rho_m)(x_k),   rho_m = rho * [material == m]
+ *
+ * where x_k are the MIDPOINTS of intervals of equal length dl laid from the
+ * point source along the straight path to the centre of detector pixel u
+ * (PAPER.md:151), dl defaults to half the smallest voxel edge,
+ * mu(x,E) = rho(x) * mu_hat(material(x), E), the energy integral
+ * is a sum over channels, the source is a spectrum phi(E) and a
+ * fluence map w(u), the detector is energy integrating with
+ * response R(E), and the geometry is the cone-beam gantry of
+ * PAPER.md:93-95.  Interpolating per-material density planes and applying
+ * mu_hat afterwards is identical to the paper's per-energy interpolation of mu
+ * by linearity of the interpolant (reading Q10).
+ *
+ * Everything runs in hand-written sm_100a CUDA kernels; there is no CPU
+ * fallback and no other backend.  Every function returns a status code and
+ * never throws or aborts across the ABI.  On error no output is written and
+ * gdrr_last_error() describes it.
+ *
+ * Memory ownership: every "_dev" pointer is DEVICE memory owned by the caller
+ * (e.g. a torch tensor) and must stay alive as documented; every other pointer
+ * is HOST memory that is copied during the call.  The library itself allocates
+ * only the small per-context tables (angles, spectrum, bowtie, fluence map,
+ * an error flag).  "cuda_stream" is a cudaStream_t passed as void* (NULL = the
+ * legacy default stream).  A context is not thread-safe; distinct contexts are
+ * independent.
+ *
+ * Units: lengths mm, rho g/cm^3, mu_hat mm^-1 per g/cm^3, mu_bt mm^-1.
+ * Conventions (readings Q1-Q9): source S = -SAD (cos phi, sin phi, 0);
+ * detector origin P = (SDD-SAD)(cos(phi+theta), sin(phi+theta), 0);
+ * u_hat = (-sin(phi+theta), cos(phi+theta), 0); v_hat = +z; pixel (i, j) centre
+ * at u = (i-(nu-1)/2) du + u_off, v = (j-(nv-1)/2) dv + v_off; voxel (ix,iy,iz)
+ * centre at centre + ((ix,iy,iz)-(N-1)/2) * spacing; clamp-to-edge inside the
+ * volume box, nothing sampled outside it.
+ */
+#ifndef GDRR_H
+#define GDRR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define GDRR_API __attribute__((visibility("default")))
+#else
+#define GDRR_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gdrr_context gdrr_context; /* geometry, spectrum tables, last error */
+typedef struct gdrr_volume gdrr_volume;   /* refers to a caller-owned device workspace */
+
+enum {
+    GDRR_OK = 0,
+    GDRR_ERR_INVALID_ARG = -1,
+    GDRR_ERR_NOT_READY = -2,   /* geometry or spectrum not set, or they disagree with the volume */
+    GDRR_ERR_CUDA = -3,
+    GDRR_ERR_WORKSPACE = -4,   /* caller's workspace too small or misaligned */
+    GDRR_ERR_UNSUPPORTED = -5
+};
+
+/* Device layout of the volume the sampler reads (step a0 of DESIGN.md).
+ * Both hold, per voxel, one fp32 per material (rho at the voxel's own material,
+ * 0 elsewhere; vector width 1, 2 or 4 floats) with a one-voxel replicated-edge
+ * pad, so clamp-to-edge costs no instruction. */
+enum {
+    GDRR_LAYOUT_BRICK = 0,  /* 2x2x2-voxel bricks, x fastest inside a brick, bricks x fastest */
+    GDRR_LAYOUT_LINEAR = 1  /* plain [nz+2][ny+2][nx+2], x fastest */
+};
+
+#define GDRR_MAX_MATERIALS 4
+#define GDRR_MAX_ENERGIES 512
+
+/* ---- context ----------------------------------------------------------- */
+
+/* Creates a context bound to CUDA device `cuda_device`.  *out is NULL on error
+ * (gdrr_last_error(NULL) then returns the message). */
+GDRR_API int gdrr_create_context(int cuda_device, gdrr_context** out);
+GDRR_API int gdrr_destroy_context(gdrr_context* ctx);
+/* Message of the last failing call on ctx (or of the last failing
+ * gdrr_create_context when ctx is NULL).  Valid until the next call. */
+GDRR_API const char* gdrr_last_error(const gdrr_context* ctx);
+
+/* ---- volume: step a0, PAPER.md:97 -------------------------------------- */
+
+/* Bytes of device workspace gdrr_create_volume needs for this shape. */
+GDRR_API int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int layout,
+                                size_t* bytes);
+
+/* Re-lays (rho, material) into the sampler's layout inside `workspace_dev`
+ * with a CUDA kernel on `cuda_stream`, checks material < n_materials on the
+ * device, and waits for that check (the only synchronising call besides the
+ * *_host variants).
+ *   rho_dev       [nz][ny][nx] fp32, x fastest, g/cm^3; borrowed for the call
+ *   material_dev  [nz][ny][nx] uint8; borrowed for the call
+ *   d*_mm         voxel edge lengths; centre_mm = centre of the volume box in
+ *                 world coordinates, NULL = the isocentre O
+ *   workspace_dev >= gdrr_volume_workspace_bytes, 256-byte aligned, must
+ *                 outlive the volume handle
+ * Errors: INVALID_ARG (dims, spacings, NULLs, a material index out of range),
+ * UNSUPPORTED (n_materials > GDRR_MAX_MATERIALS), WORKSPACE, CUDA. */
+GDRR_API int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* material_dev,
+                       int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
+                       const double centre_mm[3], int n_materials, int layout,
+                       void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                       gdrr_volume** out);
+
+/* Same, from HOST arrays: copies them into the caller's device staging buffers
+ * (rho_stage_dev: nx*ny*nz floats, material_stage_dev: nx*ny*nz bytes) on the
+ * stream, then proceeds as gdrr_create_volume. */
+GDRR_API int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host,
+                            const uint8_t* material_host,
+                            int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
+                            const double centre_mm[3], int n_materials, int layout,
+                            float* rho_stage_dev, uint8_t* material_stage_dev,
+                            void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                            gdrr_volume** out);
+
+/* Frees the handle, never the workspace. */
+GDRR_API int gdrr_destroy_volume(gdrr_volume* vol);
+
+/* ---- geometry: PAPER.md:93-95, 282 -------------------------------------- */
+
+/* sad = source-to-axis distance, sdd = source-to-detector distance (AID = sdd -
+ * sad), theta = angle between SO and OP, phi_rad[n_proj] = gantry angles
+ * (host, copied; their cos/sin are taken here with the host libm and given to
+ * the kernels as data), step_mm = dl (<= 0: half the smallest voxel edge of the
+ * volume given to gdrr_project).  Requires sdd > sad > 0, positive pixel
+ * counts and sizes, n_proj >= 1, finite values. */
+GDRR_API int gdrr_set_geometry(gdrr_context* ctx, double sad_mm, double sdd_mm, double theta_rad,
+                      int nu, int nv, double du_mm, double dv_mm,
+                      double u_offset_mm, double v_offset_mm,
+                      int n_proj, const double* phi_rad, double step_mm);
+
+/* ---- source and detector: PAPER.md:111, 117-121, 147-149 ---------------- */
+
+/*   phi_weight  [n_energy] per-channel spectrum weights, used as given
+ *   response    [n_energy] R(E)
+ *   mu_hat      [n_materials][n_energy], total over interaction types
+ *   fluence_map [nv][nu] w(u) or NULL (= 1); needs gdrr_set_geometry first
+ *   bowtie_mu   [n_energy] and bowtie_thickness_mm [nu], both or neither
+ * All host, copied.  Values must be finite. */
+GDRR_API int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,
+                      const double* phi_weight, const double* response, const double* mu_hat,
+                      const float* fluence_map, const double* bowtie_mu,
+                      const double* bowtie_thickness_mm);
+
+/* ---- projection: steps a1-a7 -------------------------------------------- */
+
+/* Projects projections [proj_begin, proj_begin + proj_count) of the geometry,
+ * asynchronously on `cuda_stream`; outputs are valid once the stream reaches
+ * this point.
+ *   signal_dev         out [proj_count][nv][nu] fp32, required
+ *   line_integrals_dev out [proj_count][n_materials][nv][nu] fp32, or NULL
+ *   ray_table_dev      out [proj_count][nv][nu][2] int32 = (j0, n): index of the
+ *                      first midpoint inside the box and the number of
+ *                      midpoints; n = 0 for a miss; or NULL
+ * Rays that miss the box get LI = 0 and the flat-field signal.
+ * Errors: NOT_READY (geometry/spectrum unset, material counts differ),
+ * INVALID_ARG (range, NULL signal, source inside the volume box), CUDA. */
+GDRR_API int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                 float* signal_dev, float* line_integrals_dev, int32_t* ray_table_dev,
+                 void* cuda_stream);
+
+/* Same, delivering the signal into HOST memory: projects in batches into the
+ * caller's device scratch `signal_stage_dev` (>= min(proj_count, stage_proj) *
+ * nv*nu floats, stage_proj >= 1 projections per batch) and copies each batch to
+ * `signal_host` [proj_count][nv][nu]; returns after the last copy completed.
+ * For overlap signal_host should be pinned. */
+GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
+                      int proj_count, float* signal_host, float* signal_stage_dev,
+                      int stage_proj, void* cuda_stream);
+
+/* Ray setup only (step a1): writes the integer ray table and/or adds the
+ * number of tri-linear samples sum(n) of the range to *n_samples_dev (a device
+ * uint64 the caller zeroed).  Either output may be NULL. */
+GDRR_API int gdrr_ray_setup(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                   int32_t* ray_table_dev, unsigned long long* n_samples_dev,
+                   void* cuda_stream);
+
+/* Number of kernels this library has launched on ctx since creation (for the
+ * harness's gpu_launches count). */
+GDRR_API unsigned long long gdrr_kernel_launches(const gdrr_context* ctx);
+
+/* Library version, "major.minor". */
+GDRR_API const char* gdrr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GDRR_H */

@@ -1,0 +1,515 @@
+// Host side of the C ABI declared in include/gdrr.h: argument validation, the
+// small context-owned device tables, and kernel launches.  No arithmetic of the
+// method happens here except what the header says is done on the host: cos/sin
+// of the gantry angles (given to the kernels as data) and table pre-scaling.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/gdrr.h"
+#include "gdrr_internal.h"
+
+using namespace gdrr;
+
+struct gdrr_context {
+    int device = 0;
+    std::string err;
+    unsigned long long launches = 0;
+    // geometry
+    bool has_geom = false;
+    double sad = 0, sdd = 0, theta = 0, du = 0, dv = 0, u_off = 0, v_off = 0, step = 0;
+    int nu = 0, nv = 0, n_proj = 0;
+    std::vector<double> phi;
+    double4* angles_dev = nullptr;
+    // spectrum
+    bool has_spec = false;
+    int n_energy = 0, n_mat = 0;
+    float4* mu_dev = nullptr;
+    float2* src_dev = nullptr;
+    float* bt_dev = nullptr;
+    float* flu_dev = nullptr;
+    // misc
+    int* flag_dev = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_done[2] = {nullptr, nullptr};
+    cudaEvent_t ev_free[2] = {nullptr, nullptr};
+};
+
+struct gdrr_volume {
+    gdrr_context* ctx;
+    void* vox;
+    int nx, ny, nz, px, py, pz;
+    double d[3], c[3];
+    int n_mat, vw, layout;
+};
+
+static thread_local std::string g_create_err;
+
+namespace {
+
+int fail(gdrr_context* ctx, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf; else g_create_err = buf;
+    return code;
+}
+
+int cuda_fail(gdrr_context* ctx, cudaError_t e, const char* what) {
+    return fail(ctx, GDRR_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+// Makes ctx's device current for the scope of one ABI call.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t status = cudaSuccess;
+    explicit DeviceGuard(int dev) {
+        status = cudaGetDevice(&prev);
+        if (status == cudaSuccess && prev != dev) {
+            status = cudaSetDevice(dev);
+            switched = (status == cudaSuccess);
+        }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+int vector_width(int n_mat) { return n_mat <= 1 ? 1 : (n_mat == 2 ? 2 : 4); }
+int padded(int n) { return (n + 2 + 1) & ~1; }
+
+bool all_finite(const double* a, size_t n) {
+    for (size_t k = 0; k < n; ++k) if (!std::isfinite(a[k])) return false;
+    return true;
+}
+
+template <class T> void free_dev(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
+
+int check_dims(gdrr_context* ctx, int nx, int ny, int nz, int n_materials, int layout) {
+    if (nx <= 0 || ny <= 0 || nz <= 0)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "volume dims must be positive (got %d %d %d)", nx, ny, nz);
+    if (n_materials <= 0)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "n_materials must be >= 1 (got %d)", n_materials);
+    if (n_materials > GDRR_MAX_MATERIALS)
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "n_materials %d > GDRR_MAX_MATERIALS %d", n_materials,
+                    GDRR_MAX_MATERIALS);
+    if (layout != GDRR_LAYOUT_BRICK && layout != GDRR_LAYOUT_LINEAR)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown layout %d", layout);
+    const double total = (double)padded(nx) * padded(ny) * padded(nz);
+    if (total >= 2147483648.0)
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "padded volume has %.0f voxels; the sampler indexes with int32", total);
+    return GDRR_OK;
+}
+
+// Fills the fp64 ray-setup parameters for (ctx geometry, volume).  Box bounds
+// are formed exactly as DESIGN.md a1 writes them: half = 0.5 * (N * d).
+int fill_geom(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+              GeomParams& g) {
+    if (!ctx->has_geom) return fail(ctx, GDRR_ERR_NOT_READY, "gdrr_set_geometry has not been called");
+    if (!vol || vol->ctx != ctx) return fail(ctx, GDRR_ERR_INVALID_ARG, "volume is NULL or belongs to another context");
+    if (proj_begin < 0 || proj_count <= 0 || proj_begin > ctx->n_proj - proj_count)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "projection range [%d, %d+%d) outside [0, %d)", proj_begin,
+                    proj_begin, proj_count, ctx->n_proj);
+    if (proj_count > 65535)
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "at most 65535 projections per call (got %d)", proj_count);
+    g.sad = ctx->sad;
+    g.aid = ctx->sdd - ctx->sad;
+    g.half_nu = 0.5 * (double)(ctx->nu - 1);
+    g.half_nv = 0.5 * (double)(ctx->nv - 1);
+    g.du = ctx->du; g.dv = ctx->dv; g.u_off = ctx->u_off; g.v_off = ctx->v_off;
+    const int n[3] = {vol->nx, vol->ny, vol->nz};
+    double dmin = vol->d[0];
+    for (int a = 0; a < 3; ++a) {
+        const double half = 0.5 * ((double)n[a] * vol->d[a]);
+        g.lo[a] = vol->c[a] - half;
+        g.hi[a] = vol->c[a] + half;
+        g.c[a] = vol->c[a];
+        g.d[a] = vol->d[a];
+        g.ofs[a] = 0.5 * (double)(n[a] - 1) + 1.0;
+        if (vol->d[a] < dmin) dmin = vol->d[a];
+    }
+    g.step = ctx->step > 0.0 ? ctx->step : 0.5 * dmin;       // PAPER.md:155, reading Q8
+    g.angles = ctx->angles_dev;
+    g.nu = ctx->nu; g.nv = ctx->nv;
+    g.proj_begin = proj_begin; g.proj_count = proj_count;
+    // the source must be outside the volume box for every requested angle
+    for (int p = proj_begin; p < proj_begin + proj_count; ++p) {
+        const double S[3] = {-(ctx->sad * std::cos(ctx->phi[p])), -(ctx->sad * std::sin(ctx->phi[p])), 0.0};
+        bool inside = true;
+        for (int a = 0; a < 3; ++a) inside = inside && S[a] >= g.lo[a] && S[a] <= g.hi[a];
+        if (inside)
+            return fail(ctx, GDRR_ERR_INVALID_ARG, "source lies inside the volume box at projection %d", p);
+    }
+    return GDRR_OK;
+}
+
+int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                 ProjectParams& P) {
+    int rc = fill_geom(ctx, vol, proj_begin, proj_count, P.g);
+    if (rc) return rc;
+    if (!ctx->has_spec) return fail(ctx, GDRR_ERR_NOT_READY, "gdrr_set_spectrum has not been called");
+    if (ctx->n_mat != vol->n_mat)
+        return fail(ctx, GDRR_ERR_NOT_READY, "spectrum has %d materials, volume has %d", ctx->n_mat, vol->n_mat);
+    P.v.vox = vol->vox;
+    if (vol->layout == GDRR_LAYOUT_BRICK) {
+        P.v.stride_y = 8 * (vol->px / 2);
+        P.v.stride_z = 8 * (vol->px / 2) * (vol->py / 2);
+    } else {
+        P.v.stride_y = vol->px;
+        P.v.stride_z = vol->px * vol->py;
+    }
+    P.mu_tab = ctx->mu_dev;
+    P.src_tab = ctx->src_dev;
+    P.bt_thick = ctx->bt_dev;
+    P.fluence = ctx->flu_dev;
+    P.n_energy = ctx->n_energy;
+    P.n_mat = ctx->n_mat;
+    // in-chunk positions are 9.23 fixed point: keep |advance| per chunk below 128 voxels
+    double dgmax = 0.0;
+    for (int a = 0; a < 3; ++a) dgmax = std::fmax(dgmax, P.g.step / vol->d[a]);
+    int chunk = kMaxChunk;
+    if (dgmax * chunk > 120.0) chunk = (int)(120.0 / dgmax);
+    if (chunk < 1)
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "step %.6g mm is more than 120 voxels long", P.g.step);
+    P.chunk = chunk;
+    return GDRR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* gdrr_version(void) { return "0.1"; }
+
+int gdrr_create_context(int cuda_device, gdrr_context** out) {
+    if (!out) return fail(nullptr, GDRR_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount");
+    if (cuda_device < 0 || cuda_device >= count)
+        return fail(nullptr, GDRR_ERR_INVALID_ARG, "cuda_device %d outside [0, %d)", cuda_device, count);
+    gdrr_context* ctx = new (std::nothrow) gdrr_context;
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "out of host memory");
+    ctx->device = cuda_device;
+    DeviceGuard guard(cuda_device);
+    if (guard.status != cudaSuccess) { delete ctx; return cuda_fail(nullptr, guard.status, "cudaSetDevice"); }
+    e = cudaMalloc(&ctx->flag_dev, sizeof(int));
+    if (e != cudaSuccess) { delete ctx; return cuda_fail(nullptr, e, "cudaMalloc(flag)"); }
+    *out = ctx;
+    return GDRR_OK;
+}
+
+int gdrr_destroy_context(gdrr_context* ctx) {
+    if (!ctx) return GDRR_OK;
+    DeviceGuard guard(ctx->device);
+    free_dev(ctx->angles_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
+    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->flag_dev);
+    for (int k = 0; k < 2; ++k) {
+        if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
+        if (ctx->ev_free[k]) cudaEventDestroy(ctx->ev_free[k]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    delete ctx;
+    return GDRR_OK;
+}
+
+const char* gdrr_last_error(const gdrr_context* ctx) {
+    return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+unsigned long long gdrr_kernel_launches(const gdrr_context* ctx) { return ctx ? ctx->launches : 0ull; }
+
+int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int layout, size_t* bytes) {
+    if (!bytes) return fail(nullptr, GDRR_ERR_INVALID_ARG, "bytes is NULL");
+    int rc = check_dims(nullptr, nx, ny, nz, n_materials, layout);
+    if (rc) return rc;
+    *bytes = (size_t)padded(nx) * padded(ny) * padded(nz) * vector_width(n_materials) * sizeof(float);
+    return GDRR_OK;
+}
+
+int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* material_dev,
+                       int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
+                       const double centre_mm[3], int n_materials, int layout,
+                       void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                       gdrr_volume** out) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!out) return fail(ctx, GDRR_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int rc = check_dims(ctx, nx, ny, nz, n_materials, layout);
+    if (rc) return rc;
+    if (!rho_dev || !material_dev) return fail(ctx, GDRR_ERR_INVALID_ARG, "rho_dev / material_dev is NULL");
+    if (!(dx_mm > 0) || !(dy_mm > 0) || !(dz_mm > 0) || !std::isfinite(dx_mm) || !std::isfinite(dy_mm) ||
+        !std::isfinite(dz_mm))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "voxel sizes must be positive and finite");
+    if (centre_mm && !all_finite(centre_mm, 3)) return fail(ctx, GDRR_ERR_INVALID_ARG, "centre_mm is not finite");
+    size_t need = 0;
+    gdrr_volume_workspace_bytes(nx, ny, nz, n_materials, layout, &need);
+    if (!workspace_dev || workspace_bytes < need)
+        return fail(ctx, GDRR_ERR_WORKSPACE, "workspace of %zu bytes given, %zu needed", workspace_bytes, need);
+    if ((uintptr_t)workspace_dev % 256)
+        return fail(ctx, GDRR_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMemsetAsync(ctx->flag_dev, 0, sizeof(int), s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(flag)");
+    IngestParams ip;
+    ip.rho = rho_dev; ip.mat = material_dev; ip.vox = workspace_dev;
+    ip.nx = nx; ip.ny = ny; ip.nz = nz;
+    ip.px = padded(nx); ip.py = padded(ny); ip.pz = padded(nz);
+    ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev;
+    const int vw = vector_width(n_materials);
+    e = launch_ingest(ip, vw, layout, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel launch");
+    ctx->launches += 1;
+    int bad = 0;
+    e = cudaMemcpyAsync(&bad, ctx->flag_dev, sizeof(int), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel");
+    if (bad) return fail(ctx, GDRR_ERR_INVALID_ARG, "a material index is >= n_materials (%d)", n_materials);
+
+    gdrr_volume* v = new (std::nothrow) gdrr_volume;
+    if (!v) return fail(ctx, GDRR_ERR_INVALID_ARG, "out of host memory");
+    v->ctx = ctx; v->vox = workspace_dev;
+    v->nx = nx; v->ny = ny; v->nz = nz; v->px = ip.px; v->py = ip.py; v->pz = ip.pz;
+    v->d[0] = dx_mm; v->d[1] = dy_mm; v->d[2] = dz_mm;
+    for (int a = 0; a < 3; ++a) v->c[a] = centre_mm ? centre_mm[a] : 0.0;
+    v->n_mat = n_materials; v->vw = vw; v->layout = layout;
+    *out = v;
+    return GDRR_OK;
+}
+
+int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host, const uint8_t* material_host,
+                            int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
+                            const double centre_mm[3], int n_materials, int layout,
+                            float* rho_stage_dev, uint8_t* material_stage_dev,
+                            void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                            gdrr_volume** out) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!out) return fail(ctx, GDRR_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int rc = check_dims(ctx, nx, ny, nz, n_materials, layout);
+    if (rc) return rc;
+    if (!rho_host || !material_host || !rho_stage_dev || !material_stage_dev)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "a host or staging pointer is NULL");
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t nvox = (size_t)nx * ny * nz;
+    cudaError_t e = cudaMemcpyAsync(rho_stage_dev, rho_host, nvox * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(material_stage_dev, material_host, nvox, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "host-to-device copy of the volume");
+    return gdrr_create_volume(ctx, rho_stage_dev, material_stage_dev, nx, ny, nz, dx_mm, dy_mm, dz_mm,
+                              centre_mm, n_materials, layout, workspace_dev, workspace_bytes, cuda_stream, out);
+}
+
+int gdrr_destroy_volume(gdrr_volume* vol) {
+    delete vol;
+    return GDRR_OK;
+}
+
+int gdrr_set_geometry(gdrr_context* ctx, double sad_mm, double sdd_mm, double theta_rad,
+                      int nu, int nv, double du_mm, double dv_mm, double u_offset_mm, double v_offset_mm,
+                      int n_proj, const double* phi_rad, double step_mm) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    const double sc[] = {sad_mm, sdd_mm, theta_rad, du_mm, dv_mm, u_offset_mm, v_offset_mm, step_mm};
+    if (!all_finite(sc, 8)) return fail(ctx, GDRR_ERR_INVALID_ARG, "a geometry scalar is not finite");
+    if (!(sad_mm > 0) || !(sdd_mm > sad_mm))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "need sdd > sad > 0 (got sad %g, sdd %g)", sad_mm, sdd_mm);
+    if (nu <= 0 || nv <= 0 || !(du_mm > 0) || !(dv_mm > 0))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "detector pixel counts and sizes must be positive");
+    if (n_proj <= 0 || !phi_rad) return fail(ctx, GDRR_ERR_INVALID_ARG, "need n_proj >= 1 and phi_rad");
+    if (!all_finite(phi_rad, (size_t)n_proj)) return fail(ctx, GDRR_ERR_INVALID_ARG, "a gantry angle is not finite");
+
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    // cos/sin once, on the host, passed to the kernels as data (DESIGN.md a1)
+    std::vector<double4> ang((size_t)n_proj);
+    for (int p = 0; p < n_proj; ++p) {
+        const double phi = phi_rad[p], psi = phi + theta_rad;
+        ang[p] = make_double4(std::cos(phi), std::sin(phi), std::cos(psi), std::sin(psi));
+    }
+    double4* dev = nullptr;
+    cudaError_t e = cudaMalloc(&dev, sizeof(double4) * (size_t)n_proj);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMalloc(angles)");
+    e = cudaMemcpy(dev, ang.data(), sizeof(double4) * (size_t)n_proj, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(dev); return cuda_fail(ctx, e, "cudaMemcpy(angles)"); }
+    if (ctx->has_geom && (nu != ctx->nu || nv != ctx->nv)) {
+        // tables shaped by the old detector are no longer valid
+        free_dev(ctx->flu_dev); free_dev(ctx->bt_dev);
+        ctx->has_spec = false;
+    }
+    free_dev(ctx->angles_dev);
+    ctx->angles_dev = dev;
+    ctx->sad = sad_mm; ctx->sdd = sdd_mm; ctx->theta = theta_rad;
+    ctx->nu = nu; ctx->nv = nv; ctx->du = du_mm; ctx->dv = dv_mm;
+    ctx->u_off = u_offset_mm; ctx->v_off = v_offset_mm;
+    ctx->n_proj = n_proj; ctx->step = step_mm;
+    ctx->phi.assign(phi_rad, phi_rad + n_proj);
+    ctx->has_geom = true;
+    return GDRR_OK;
+}
+
+int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,
+                      const double* phi_weight, const double* response, const double* mu_hat,
+                      const float* fluence_map, const double* bowtie_mu,
+                      const double* bowtie_thickness_mm) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (n_energy <= 0 || n_energy > GDRR_MAX_ENERGIES)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "n_energy must be in [1, %d] (got %d)", GDRR_MAX_ENERGIES, n_energy);
+    if (n_materials <= 0) return fail(ctx, GDRR_ERR_INVALID_ARG, "n_materials must be >= 1");
+    if (n_materials > GDRR_MAX_MATERIALS)
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "n_materials %d > GDRR_MAX_MATERIALS %d", n_materials, GDRR_MAX_MATERIALS);
+    if (!phi_weight || !response || !mu_hat) return fail(ctx, GDRR_ERR_INVALID_ARG, "a table pointer is NULL");
+    if ((bowtie_mu == nullptr) != (bowtie_thickness_mm == nullptr))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "bowtie_mu and bowtie_thickness_mm go together");
+    if ((fluence_map || bowtie_mu) && !ctx->has_geom)
+        return fail(ctx, GDRR_ERR_NOT_READY, "fluence map / bowtie need gdrr_set_geometry first (detector shape)");
+    if (!all_finite(phi_weight, n_energy) || !all_finite(response, n_energy) ||
+        !all_finite(mu_hat, (size_t)n_energy * n_materials) ||
+        (bowtie_mu && (!all_finite(bowtie_mu, n_energy) || !all_finite(bowtie_thickness_mm, ctx->nu))))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "a table entry is not finite");
+    if (fluence_map) {
+        const size_t n = (size_t)ctx->nu * ctx->nv;
+        for (size_t k = 0; k < n; ++k)
+            if (!std::isfinite(fluence_map[k])) return fail(ctx, GDRR_ERR_INVALID_ARG, "fluence map entry is not finite");
+    }
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+
+    // exp(-tau) is evaluated as exp2(-log2(e) * tau): fold log2(e) into the tables
+    const double log2e = 1.4426950408889634074;
+    std::vector<float4> mu((size_t)n_energy);
+    std::vector<float2> src((size_t)n_energy);
+    for (int e = 0; e < n_energy; ++e) {
+        float m4[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int m = 0; m < n_materials; ++m) m4[m] = (float)(log2e * mu_hat[(size_t)m * n_energy + e]);
+        mu[e] = make_float4(m4[0], m4[1], m4[2], m4[3]);
+        src[e] = make_float2((float)(phi_weight[e] * response[e]), bowtie_mu ? (float)(log2e * bowtie_mu[e]) : 0.f);
+    }
+    float4* mu_dev = nullptr; float2* src_dev = nullptr; float* bt_dev = nullptr; float* flu_dev = nullptr;
+    cudaError_t e = cudaMalloc(&mu_dev, sizeof(float4) * n_energy);
+    if (e == cudaSuccess) e = cudaMalloc(&src_dev, sizeof(float2) * n_energy);
+    if (e == cudaSuccess) e = cudaMemcpy(mu_dev, mu.data(), sizeof(float4) * n_energy, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(src_dev, src.data(), sizeof(float2) * n_energy, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && bowtie_mu) {
+        std::vector<float> bt((size_t)ctx->nu);
+        for (int i = 0; i < ctx->nu; ++i) bt[i] = (float)bowtie_thickness_mm[i];
+        e = cudaMalloc(&bt_dev, sizeof(float) * ctx->nu);
+        if (e == cudaSuccess) e = cudaMemcpy(bt_dev, bt.data(), sizeof(float) * ctx->nu, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess && fluence_map) {
+        const size_t n = (size_t)ctx->nu * ctx->nv;
+        e = cudaMalloc(&flu_dev, sizeof(float) * n);
+        if (e == cudaSuccess) e = cudaMemcpy(flu_dev, fluence_map, sizeof(float) * n, cudaMemcpyHostToDevice);
+    }
+    if (e != cudaSuccess) {
+        free_dev(mu_dev); free_dev(src_dev); free_dev(bt_dev); free_dev(flu_dev);
+        return cuda_fail(ctx, e, "uploading the spectrum tables");
+    }
+    free_dev(ctx->mu_dev); free_dev(ctx->src_dev); free_dev(ctx->bt_dev); free_dev(ctx->flu_dev);
+    ctx->mu_dev = mu_dev; ctx->src_dev = src_dev; ctx->bt_dev = bt_dev; ctx->flu_dev = flu_dev;
+    ctx->n_energy = n_energy; ctx->n_mat = n_materials;
+    ctx->has_spec = true;
+    return GDRR_OK;
+}
+
+int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                 float* signal_dev, float* line_integrals_dev, int32_t* ray_table_dev,
+                 void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!signal_dev) return fail(ctx, GDRR_ERR_INVALID_ARG, "signal_dev is NULL");
+    ProjectParams P;
+    int rc = fill_project(ctx, vol, proj_begin, proj_count, P);
+    if (rc) return rc;
+    P.signal = signal_dev; P.li = line_integrals_dev; P.ray_table = ray_table_dev;
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaError_t e = launch_project(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "project kernel launch");
+    ctx->launches += 1;
+    return GDRR_OK;
+}
+
+int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                      float* signal_host, float* signal_stage_dev, int stage_proj, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!signal_host || !signal_stage_dev || stage_proj < 1)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "signal_host / signal_stage_dev is NULL or stage_proj < 1");
+    ProjectParams P;
+    int rc = fill_project(ctx, vol, proj_begin, proj_count, P);
+    if (rc) return rc;
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSuccess;
+    if (!ctx->copy_stream) {
+        e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+        for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+            e = cudaEventCreateWithFlags(&ctx->ev_done[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_free[k], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "creating the copy stream");
+    }
+    // two half-buffers: the kernel fills one while the other drains to the host
+    const size_t plane = (size_t)ctx->nu * ctx->nv;
+    const int slots = stage_proj >= 2 ? 2 : 1;
+    const int batch = stage_proj / slots;
+    int used[2] = {0, 0};
+    int done = 0;
+    for (int b = 0; done < proj_count; ++b) {
+        const int slot = b % slots;
+        const int cnt = proj_count - done < batch ? proj_count - done : batch;
+        float* stage = signal_stage_dev + (size_t)slot * batch * plane;
+        if (used[slot]) e = cudaStreamWaitEvent(s, ctx->ev_free[slot], 0);
+        if (e != cudaSuccess) break;
+        ProjectParams Pb = P;
+        Pb.g.proj_begin = proj_begin + done;
+        Pb.g.proj_count = cnt;
+        Pb.signal = stage; Pb.li = nullptr; Pb.ray_table = nullptr;
+        e = launch_project(Pb, vol->vw, vol->layout, s);
+        if (e != cudaSuccess) break;
+        ctx->launches += 1;
+        e = cudaEventRecord(ctx->ev_done[slot], s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_done[slot], 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(signal_host + (size_t)done * plane, stage, sizeof(float) * plane * cnt,
+                                cudaMemcpyDeviceToHost, ctx->copy_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_free[slot], ctx->copy_stream);
+        if (e != cudaSuccess) break;
+        used[slot] = 1;
+        done += cnt;
+    }
+    cudaError_t e2 = cudaStreamSynchronize(ctx->copy_stream);
+    if (e == cudaSuccess) e = e2;
+    // later work on the caller's stream must not overtake the drains either
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gdrr_project_host");
+    return GDRR_OK;
+}
+
+int gdrr_ray_setup(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                   int32_t* ray_table_dev, unsigned long long* n_samples_dev, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!ray_table_dev && !n_samples_dev)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "both outputs are NULL");
+    GeomParams g;
+    int rc = fill_geom(ctx, vol, proj_begin, proj_count, g);
+    if (rc) return rc;
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaError_t e = launch_ray_setup(g, ray_table_dev, n_samples_dev, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "ray-setup kernel launch");
+    ctx->launches += 1;
+    return GDRR_OK;
+}
+
+}  // extern "C"

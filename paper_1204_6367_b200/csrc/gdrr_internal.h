@@ -1,0 +1,69 @@
+// Internal declarations shared by the translation units of libgdrr_b200.so.
+// Not part of the ABI (include/gdrr.h is).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gdrr {
+
+// Tile of detector pixels one CTA owns: 16 x 16, eight warps of 8 (u) x 4 (v)
+// pixels each.  A warp's rays then cross the volume as a beam about 4 x 1.6
+// voxels wide at C3.
+constexpr int kTileU = 16;
+constexpr int kTileV = 16;
+constexpr int kThreads = kTileU * kTileV;
+constexpr int kMaxChunk = 32;       // samples between two fp64 re-bases of the position
+constexpr int kFracBits = 23;       // fixed-point fraction bits of the in-chunk position
+
+// Everything the ray-setup arithmetic (step a1) needs.  All fp64; the order of
+// operations in ray_setup.cuh is part of the definition of (j0, n).
+struct GeomParams {
+    double sad, aid;                // source-to-axis, axis-to-imager (= sdd - sad)
+    double half_nu, half_nv;        // 0.5 * (nu - 1), 0.5 * (nv - 1)
+    double du, dv, u_off, v_off;
+    double step;                    // dl
+    double lo[3], hi[3];            // volume box
+    double c[3], d[3];              // box centre, voxel size
+    double ofs[3];                  // 0.5 * (N - 1) + 1: world -> padded index coordinates
+    const double4* angles;          // [n_proj] (cos phi, sin phi, cos psi, sin psi), device
+    int nu, nv;
+    int proj_begin, proj_count;
+};
+
+struct VolumeParams {
+    const void* vox;                // device, layout below
+    int stride_y;                   // BRICK: 8 * bricks per row;      LINEAR: padded nx
+    int stride_z;                   // BRICK: 8 * bricks per slab;     LINEAR: padded nx * ny
+};
+
+struct ProjectParams {
+    GeomParams g;
+    VolumeParams v;
+    const float4* mu_tab;           // [n_energy] log2(e) * mu_hat[m = 0..3][E]
+    const float2* src_tab;          // [n_energy] (phi_E * R_E, log2(e) * mu_bt[E])
+    const float* bt_thick;          // [nu] or nullptr
+    const float* fluence;           // [nv][nu] or nullptr
+    int n_energy, n_mat;
+    int chunk;                      // <= kMaxChunk
+    float* signal;                  // [proj_count][nv][nu]
+    float* li;                      // [proj_count][n_mat][nv][nu] or nullptr
+    int32_t* ray_table;             // [proj_count][nv][nu][2] or nullptr
+};
+
+struct IngestParams {
+    const float* rho;               // [nz][ny][nx]
+    const uint8_t* mat;
+    void* vox;
+    int nx, ny, nz;
+    int px, py, pz;                 // stored dims: N + 2 rounded up to even
+    int n_mat;
+    int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
+};
+
+// Host-callable launchers (each returns the cudaGetLastError() of its launch).
+cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
+cudaError_t launch_project(const ProjectParams& p, int vw, int layout, cudaStream_t s);
+cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
+                             unsigned long long* n_samples, cudaStream_t s);
+
+}  // namespace gdrr

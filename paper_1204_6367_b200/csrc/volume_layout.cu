@@ -1,0 +1,84 @@
+// Step a0: volume ingest ("material type and density at each voxel").
+//
+// Turns (rho fp32, material u8) [nz][ny][nx] into the layout the sampler reads:
+// per voxel VW floats (rho in the slot of the voxel's material, 0 elsewhere),
+// with a one-voxel replicated-edge pad (so clamp-to-edge, reading Q7, needs no
+// instruction in the sampler), stored either as 2x2x2 bricks or linearly.
+// One thread per stored voxel, stores coalesced in storage order.
+#include "gdrr_internal.h"
+
+namespace gdrr {
+
+template <int VW> struct VoxT;
+template <> struct VoxT<1> { using T = float; };
+template <> struct VoxT<2> { using T = float2; };
+template <> struct VoxT<4> { using T = float4; };
+
+template <int VW>
+__device__ __forceinline__ typename VoxT<VW>::T one_hot(float rho, int m);
+template <> __device__ __forceinline__ float one_hot<1>(float rho, int) { return rho; }
+template <> __device__ __forceinline__ float2 one_hot<2>(float rho, int m) {
+    return make_float2(m == 0 ? rho : 0.f, m == 1 ? rho : 0.f);
+}
+template <> __device__ __forceinline__ float4 one_hot<4>(float rho, int m) {
+    return make_float4(m == 0 ? rho : 0.f, m == 1 ? rho : 0.f, m == 2 ? rho : 0.f,
+                       m == 3 ? rho : 0.f);
+}
+
+template <int VW, int LAYOUT>
+__global__ void __launch_bounds__(256)
+gdrr_ingest_kernel(const IngestParams P) {
+    using V = typename VoxT<VW>::T;
+    const size_t total = (size_t)P.px * P.py * P.pz;
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= total) return;
+    int sx_, sy_, sz_;      // stored (padded) coordinates of element o
+    if (LAYOUT == 0) {
+        const int e = (int)(o & 7);
+        size_t b = o >> 3;
+        const int nbx = P.px >> 1, nby = P.py >> 1;
+        const int bx = (int)(b % nbx);
+        b /= nbx;
+        const int by = (int)(b % nby);
+        const int bz = (int)(b / nby);
+        sx_ = 2 * bx + (e & 1);
+        sy_ = 2 * by + ((e >> 1) & 1);
+        sz_ = 2 * bz + (e >> 2);
+    } else {
+        size_t t = o;
+        sx_ = (int)(t % P.px);
+        t /= P.px;
+        sy_ = (int)(t % P.py);
+        sz_ = (int)(t / P.py);
+    }
+    // stored index s <-> voxel s - 1, clamped to the lattice (replicated edge)
+    const int ix = min(max(sx_ - 1, 0), P.nx - 1);
+    const int iy = min(max(sy_ - 1, 0), P.ny - 1);
+    const int iz = min(max(sz_ - 1, 0), P.nz - 1);
+    const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
+    const float rho = P.rho[src];
+    const int m = P.mat[src];
+    if (m >= P.n_mat) *P.bad_flag = 1;
+    reinterpret_cast<V*>(P.vox)[o] = one_hot<VW>(rho, m);
+}
+
+template <int VW, int LAYOUT>
+static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
+    const size_t total = (size_t)p.px * p.py * p.pz;
+    const unsigned int blocks = (unsigned int)((total + 255) / 256);
+    gdrr_ingest_kernel<VW, LAYOUT><<<blocks, 256, 0, s>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s) {
+    if (layout == 0) {
+        if (vw == 1) return launch_ingest_t<1, 0>(p, s);
+        if (vw == 2) return launch_ingest_t<2, 0>(p, s);
+        return launch_ingest_t<4, 0>(p, s);
+    }
+    if (vw == 1) return launch_ingest_t<1, 1>(p, s);
+    if (vw == 2) return launch_ingest_t<2, 1>(p, s);
+    return launch_ingest_t<4, 1>(p, s);
+}
+
+}  // namespace gdrr
