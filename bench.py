@@ -1,0 +1,359 @@
+"""Benchmark of the gDRR primary-signal projector on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl reference]
+
+One "step" is one pass of the whole hot path over one synthetic scan: volume
+ingest (a0) from device-resident (rho, material), then ray setup, tri-linear
+sampling, energy sum and store (a1-a7) for every projection of the workload.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "trilinear_samples_per_s"
+UNIT = "samples/s"
+SM_COUNT = 148
+L1_BYTES_PER_CLK = 128          # per SM, DESIGN.md "Roofline"
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)),
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for row in self.rows:
+            parts = [p.strip() for p in row.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "power_w_max": float(max(power)) if power else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_config(w, name, world, n_total, launch_proj):
+    nx, ny, nz = w.dims
+    return {"workload": name, "volume": [nx, ny, nz], "voxel_mm": list(w.spacing),
+            "materials": w.n_materials, "energy_bins": w.n_energy, "detector": [w.nu, w.nv],
+            "pixel_mm": w.du, "step_mm": w.step_mm, "projections_per_gpu": w.n_proj,
+            "projections_total": n_total, "projections_per_launch": launch_proj,
+            "parallelism": f"projection-sharded x{world}, no collective",
+            "l2": "volume in device layout exceeds L2 (no flush needed)" if
+                  (nx + 2) * (ny + 2) * (nz + 2) * 4 * (1 if w.n_materials == 1 else 2 if w.n_materials == 2 else 4)
+                  > 126e6 else "L2 flushed between steps"}
+
+
+# ---------------------------------------------------------------------------
+# the reference arm and the cpu_baseline leg: the oracle, as it stands
+# ---------------------------------------------------------------------------
+
+def oracle_sample(w, rows, projection):
+    """Pixel list: `rows` evenly spaced detector rows of one projection."""
+    jj = np.linspace(0, w.nv - 1, rows).round().astype(np.int32)
+    ii = np.arange(w.nu, dtype=np.int32)
+    J, I = np.meshgrid(jj, ii, indexing="ij")
+    return np.stack([np.full(J.size, projection, dtype=np.int32), I.ravel(), J.ravel()], axis=1)
+
+
+def time_oracle(w, pix):
+    import oracle
+    t0 = time.perf_counter()
+    out = oracle.project(w, pixels=pix, want_li=False)
+    dt = time.perf_counter() - t0
+    return int(out["ray_table"][:, 1].sum()), dt, oracle.n_threads_available()
+
+
+def sized_oracle_sample(w, seconds):
+    """A pixel list of the workload worth about `seconds` of oracle time on this
+    host: probe the rate on 16 rows of one projection, then take whole
+    projections evenly spaced over the scan (or fewer rows of one projection)."""
+    p = min(37, w.n_proj - 1)
+    probe_rows = max(1, min(w.nv, 16))
+    time_oracle(w, oracle_sample(w, probe_rows, p))            # touch the volume once
+    n, dt, _ = time_oracle(w, oracle_sample(w, probe_rows, p))
+    per_proj = n * (w.nv / probe_rows)
+    want = max(1.0, seconds * (n / dt))
+    n_proj = int(min(w.n_proj, max(1, round(want / per_proj))))
+    if want >= per_proj:
+        projs = np.linspace(0, w.n_proj - 1, n_proj).round().astype(int)
+        pix = np.concatenate([oracle_sample(w, w.nv, int(q)) for q in projs])
+        return pix, f"all {w.nv} x {w.nu} pixels of {n_proj} projection(s) evenly spaced over the scan"
+    rows = int(max(1, min(w.nv, round(w.nv * want / per_proj))))
+    return oracle_sample(w, rows, p), f"{rows} evenly spaced detector rows x {w.nu} columns of projection {p}"
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from workloads import make_workload
+    w = make_workload(args.workload)
+    pix, sample = sized_oracle_sample(w, args.ref_seconds)
+    for _ in range(args.warmup):
+        time_oracle(w, pix[: max(1, len(pix) // 16)])
+    total, elapsed, cores = 0, 0.0, 1
+    for _ in range(args.steps):
+        n, dt, cores = time_oracle(w, pix)
+        total += n
+        elapsed += dt
+    value = total / elapsed
+    per_proj = n * (w.nu * w.nv / len(pix))
+    sample = f"{sample}, per step"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * elapsed / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
+            "config": workload_config(w, args.workload, 1, w.n_proj, 0),
+            "projections_per_s": value / per_proj,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------
+# the B200 arm
+# ---------------------------------------------------------------------------
+
+def run_b200(args):
+    import torch
+    import paper_1204_6367_b200 as g
+    from paper_1204_6367_b200 import dist as gd
+    from workloads import make_workload
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU path")
+    rank, local_rank, world = gd.init_process_group("nccl")
+    if world != args.gpus:
+        raise RuntimeError(f"--gpus {args.gpus} but WORLD_SIZE is {world}")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    peaks = measured_peaks()
+
+    # the N-GPU job is one scan of n_proj * N evenly spaced angles, sharded by projection
+    w0 = make_workload(args.workload)
+    per_gpu = w0.n_proj if args.projections <= 0 else args.projections
+    n_total = per_gpu * world
+    mine = gd.strided_shard(n_total, world, rank)
+    w = w0.with_phis(gd.scan_angles(n_total)[mine])
+    launch_proj = per_gpu if args.launch_proj <= 0 else min(args.launch_proj, per_gpu)
+
+    pr = g.Projector(w, device=local_rank, layout=args.layout)
+    signal = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+    n_samples = pr.count_samples()
+    ingest_launches_before = pr.kernel_launches()
+
+    vw = 1 if w.n_materials == 1 else 2 if w.n_materials == 2 else 4
+    nx, ny, nz = w.dims
+    vol_bytes = (nx + 2) * (ny + 2) * (nz + 2) * 4 * vw
+    flush = (torch.empty(256 << 20, dtype=torch.uint8, device=dev) if vol_bytes <= 126e6 else None)
+
+    def step(events=None):
+        if flush is not None:                              # inputs fit in L2: evict them
+            flush.zero_()
+        if events is not None:
+            events[2].record(stream)
+        pr.ingest()                                        # a0
+        if events is not None:
+            events[0].record(stream)
+        for b in range(0, per_gpu, launch_proj):            # a1-a7
+            cnt = min(launch_proj, per_gpu - b)
+            g.gdrr_project(pr.ctx, pr.vol, b, cnt, signal[b:b + cnt])
+        if events is not None:
+            events[1].record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    kev = [tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(args.steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = pr.kernel_launches()
+    gd.barrier()
+    torch.cuda.synchronize()
+    t_begin.record(stream)
+    for k in range(args.steps):
+        step(kev[k])
+    t_end.record(stream)
+    torch.cuda.synchronize()
+    gd.barrier()
+    launches = pr.kernel_launches() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    bracket_ms = t_begin.elapsed_time(t_end)
+    if flush is not None:                                   # leave the L2 flushes out of the step time
+        bracket_ms = float(np.sum([c.elapsed_time(b) for a, b, c in kev]))
+    elapsed_ms = gd.max_over_ranks(bracket_ms, dev)
+    kernel_ms = float(np.mean([a.elapsed_time(b) for a, b, c in kev]))     # all project launches of a step
+    total_samples = gd.sum_over_ranks(n_samples, dev)
+    checksum = float(signal.double().sum().item())
+
+    value = total_samples * args.steps / (elapsed_ms * 1e-3)
+    proj_per_s = n_total * args.steps / (elapsed_ms * 1e-3)
+
+    # ---- e2e: the same step through the host-buffer entry points ------------------
+    e2e = None
+    if not args.no_e2e:
+        rho_h = torch.from_numpy(w.rho).pin_memory()
+        mat_h = torch.from_numpy(w.mat).pin_memory()
+        out_h = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32).pin_memory()
+        stage_proj = min(per_gpu, 32)
+        stage = torch.empty((stage_proj, w.nv, w.nu), dtype=torch.float32, device=dev)
+
+        def e2e_step():
+            pr.ingest_host(rho_h, mat_h)
+            g.gdrr_project_host(pr.ctx, pr.vol, 0, per_gpu, out_h, stage, stage_proj)
+
+        e2e_step()
+        torch.cuda.synchronize()
+        gd.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e2e_step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        gd.barrier()
+        e2e_ms = gd.max_over_ranks(max(e0.elapsed_time(e1), wall_ms), dev)
+        same = bool(torch.equal(out_h, signal.cpu()))
+        e2e = {"value": total_samples * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+               "projections_per_s": n_total * args.steps / (e2e_ms * 1e-3),
+               "ms_per_step": e2e_ms / args.steps,
+               "h2d_bytes_per_step": int(rho_h.numel() * 4 + mat_h.numel()),
+               "d2h_bytes_per_step": int(out_h.numel() * 4),
+               "bit_identical_to_device_path": same,
+               "api": "gdrr_create_volume_host + gdrr_project_host (pinned host buffers)"}
+
+    if rank != 0:
+        pr.close()
+        return
+
+    # ---- roofline of the dominant kernel (gdrr_project_kernel) ----------------------
+    l1_bytes = 8 * vw * 4 * n_samples                       # 8 corner vectors per sample
+    l1_peak = SM_COUNT * L1_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9       # GB/s
+    l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
+    hbm_bytes = per_gpu * (vol_bytes + w.nu * w.nv * 4)
+    hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
+    ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
+    roofline = {"kernel": "gdrr_project_kernel", "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
+                "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
+                "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),
+                "peak_def": f"{SM_COUNT} SMs x {L1_BYTES_PER_CLK} B/clk x {peaks['sm_max_mhz']:.0f} MHz (max SM clock)",
+                "algorithmic": f"8 corners x {vw} floats x 4 B = {32 * vw} B per sample through L1",
+                "samples_per_clk_per_sm": n_samples / (kernel_ms * 1e-3) / (SM_COUNT * peaks["sm_max_mhz"] * 1e6),
+                "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
+                        "algorithmic": "device-layout volume once per projection + 4 B per pixel"}}
+
+    # ---- cpu_baseline: the oracle on a bounded sample of the same workload -----------
+    cpu = None
+    if not args.no_cpu_baseline:
+        pix, sample = sized_oracle_sample(w, args.cpu_seconds)
+        n, dt, cores = time_oracle(w, pix)
+        cpu = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": f"{sample} ({n} samples)"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
+            "config": workload_config(w, args.workload, world, n_total, launch_proj),
+            "projections_per_s": proj_per_s, "samples_per_step": total_samples,
+            "paper_context": "paper: 1.2-2.3 s per poly-energetic projection on a GTX 580 (PAPER.md:366-367)",
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu, "checksum": checksum, "library": g.LIBRARY_PATH}
+    print(json.dumps(line), flush=True)
+    pr.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--projections", type=int, default=0, help="projections per GPU (0 = the workload's)")
+    ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
+    ap.add_argument("--layout", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
+    ap.add_argument("--ref-seconds", type=float, default=8.0, help="target oracle time per step of --impl reference")
+    ap.add_argument("--ncu-dram-bytes", type=float, default=0.0,
+                    help="dram bytes per launch from the committed ncu capture (profiles/)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -176,7 +176,7 @@ def test_edge_cases(gdrr, case, layout):
         shape, spacing = (9, 13, 17), (1.3, 2.1, 3.7)
         kw.update(centre=(12.0, -7.5, 4.0), nu=50, nv=40)
     elif case == "theta_offset":
-        kw.update(theta=math.radians(9.0))
+        kw.update(theta=math.radians(9.0), nu=61, du=4.0)
     elif case == "three_materials":
         n_mat = 3
     elif case == "long_step":
