@@ -207,7 +207,7 @@ def run_b200(args):
 
     vw = 1 if w.n_materials == 1 else 2 if w.n_materials == 2 else 4
     nx, ny, nz = w.dims
-    vol_bytes = (nx + 2) * (ny + 2) * (nz + 2) * 4 * vw
+    vol_bytes = (nx + 2) * (ny + 2) * (nz + 2) * (16 if args.layout == 2 else 4 * vw)
     flush = (torch.empty(256 << 20, dtype=torch.uint8, device=dev) if vol_bytes <= 126e6 else None)
 
     def step(events=None):
@@ -295,17 +295,18 @@ def run_b200(args):
         return
 
     # ---- roofline of the dominant kernel (gdrr_project_kernel) ----------------------
-    l1_bytes = 8 * vw * 4 * n_samples                       # 8 corner vectors per sample
+    corner_bytes = 4 if args.layout == 2 else 4 * vw        # packed word, or one float per material
+    l1_bytes = 8 * corner_bytes * n_samples                 # 8 corners per sample
     l1_peak = SM_COUNT * L1_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9       # GB/s
     l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
     hbm_bytes = per_gpu * (vol_bytes + w.nu * w.nv * 4)
     hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
-    roofline = {"kernel": "gdrr_project_kernel", "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
+    roofline = {"kernel": "gdrr_project_packed_kernel" if args.layout == 2 else "gdrr_project_kernel", "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
                 "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
                 "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),
                 "peak_def": f"{SM_COUNT} SMs x {L1_BYTES_PER_CLK} B/clk x {peaks['sm_max_mhz']:.0f} MHz (max SM clock)",
-                "algorithmic": f"8 corners x {vw} floats x 4 B = {32 * vw} B per sample through L1",
+                "algorithmic": f"8 corners x {corner_bytes} B = {8 * corner_bytes} B per sample through L1",
                 "samples_per_clk_per_sm": n_samples / (kernel_ms * 1e-3) / (SM_COUNT * peaks["sm_max_mhz"] * 1e6),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
@@ -341,7 +342,7 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--projections", type=int, default=0, help="projections per GPU (0 = the workload's)")
     ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
-    ap.add_argument("--layout", type=int, default=0)
+    ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")

@@ -68,13 +68,18 @@ enum {
     GDRR_ERR_UNSUPPORTED = -5
 };
 
-/* Device layout of the volume the sampler reads (step a0 of DESIGN.md).
- * Both hold, per voxel, one fp32 per material (rho at the voxel's own material,
- * 0 elsewhere; vector width 1, 2 or 4 floats) with a one-voxel replicated-edge
- * pad, so clamp-to-edge costs no instruction. */
+/* Device layout of the volume the sampler reads (step a0 of DESIGN.md).  All
+ * carry a one-voxel replicated-edge pad, so clamp-to-edge costs no instruction.
+ * BRICK and LINEAR hold, per voxel, one fp32 per material (rho at the voxel's
+ * own material, 0 elsewhere; vector width 1, 2 or 4 floats), rho bit-exact.
+ * PACKED_QUAD (the fast one) holds one 32-bit word per voxel -- fp32 rho rounded
+ * to a 22-bit mantissa with the material index in the two freed bits when
+ * n_materials > 1 (|stored - rho| <= 5 ulp = 3e-7 relative) -- as overlapping
+ * 2x2 (x, y) quads, 16 bytes per voxel. */
 enum {
-    GDRR_LAYOUT_BRICK = 0,  /* 2x2x2-voxel bricks, x fastest inside a brick, bricks x fastest */
-    GDRR_LAYOUT_LINEAR = 1  /* plain [nz+2][ny+2][nx+2], x fastest */
+    GDRR_LAYOUT_BRICK = 0,       /* 2x2x2-voxel bricks, x fastest inside a brick, bricks x fastest */
+    GDRR_LAYOUT_LINEAR = 1,      /* plain [nz+2][ny+2][nx+2], x fastest */
+    GDRR_LAYOUT_PACKED_QUAD = 2  /* quads of packed words, 4x2 tiles per slab, slabs linear */
 };
 
 #define GDRR_MAX_MATERIALS 4

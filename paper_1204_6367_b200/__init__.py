@@ -26,6 +26,7 @@ GDRR_ERR_WORKSPACE = -4
 GDRR_ERR_UNSUPPORTED = -5
 GDRR_LAYOUT_BRICK = 0
 GDRR_LAYOUT_LINEAR = 1
+GDRR_LAYOUT_PACKED_QUAD = 2
 GDRR_MAX_MATERIALS = 4
 GDRR_MAX_ENERGIES = 512
 
@@ -138,7 +139,7 @@ def gdrr_last_error(ctx=None):
     return msg.decode() if msg else ""
 
 
-def gdrr_volume_workspace_bytes(nx, ny, nz, n_materials, layout=GDRR_LAYOUT_BRICK):
+def gdrr_volume_workspace_bytes(nx, ny, nz, n_materials, layout=GDRR_LAYOUT_PACKED_QUAD):
     out = ctypes.c_size_t()
     _check(_lib.gdrr_volume_workspace_bytes(nx, ny, nz, n_materials, layout, ctypes.byref(out)))
     return out.value
@@ -259,7 +260,7 @@ class Projector:
     """Context + volume + the torch tensors they borrow, built from a
     workload-like object (attributes as workloads.Workload)."""
 
-    def __init__(self, w, device=0, layout=GDRR_LAYOUT_BRICK, from_host=False):
+    def __init__(self, w, device=0, layout=GDRR_LAYOUT_PACKED_QUAD, from_host=False):
         import torch
         self.torch = torch
         self.device = torch.device("cuda", device)

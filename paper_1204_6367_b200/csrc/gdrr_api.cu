@@ -81,7 +81,24 @@ struct DeviceGuard {
 };
 
 int vector_width(int n_mat) { return n_mat <= 1 ? 1 : (n_mat == 2 ? 2 : 4); }
-int padded(int n) { return (n + 2 + 1) & ~1; }
+
+// Stored dims of the device volume: voxels N + 2 rounded up to even (BRICK, LINEAR);
+// quads (N + 1 rounded up to the 4 x 2 tile) x (N + 2 slabs) for PACKED_QUAD.
+void stored_dims(int nx, int ny, int nz, int layout, int& px, int& py, int& pz) {
+    if (layout == GDRR_LAYOUT_PACKED_QUAD) {
+        px = (nx + 1 + 3) & ~3;
+        py = (ny + 1 + 1) & ~1;
+        pz = nz + 2;
+    } else {
+        px = (nx + 3) & ~1;
+        py = (ny + 3) & ~1;
+        pz = (nz + 3) & ~1;
+    }
+}
+
+size_t element_bytes(int n_mat, int layout) {
+    return layout == GDRR_LAYOUT_PACKED_QUAD ? 16 : vector_width(n_mat) * sizeof(float);
+}
 
 bool all_finite(const double* a, size_t n) {
     for (size_t k = 0; k < n; ++k) if (!std::isfinite(a[k])) return false;
@@ -98,9 +115,11 @@ int check_dims(gdrr_context* ctx, int nx, int ny, int nz, int n_materials, int l
     if (n_materials > GDRR_MAX_MATERIALS)
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "n_materials %d > GDRR_MAX_MATERIALS %d", n_materials,
                     GDRR_MAX_MATERIALS);
-    if (layout != GDRR_LAYOUT_BRICK && layout != GDRR_LAYOUT_LINEAR)
+    if (layout != GDRR_LAYOUT_BRICK && layout != GDRR_LAYOUT_LINEAR && layout != GDRR_LAYOUT_PACKED_QUAD)
         return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown layout %d", layout);
-    const double total = (double)padded(nx) * padded(ny) * padded(nz);
+    int px, py, pz;
+    stored_dims(nx, ny, nz, layout, px, py, pz);
+    const double total = (double)px * py * pz;
     if (total >= 2147483648.0)
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "padded volume has %.0f voxels; the sampler indexes with int32", total);
     return GDRR_OK;
@@ -159,6 +178,9 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     if (vol->layout == GDRR_LAYOUT_BRICK) {
         P.v.stride_y = 8 * (vol->px / 2);
         P.v.stride_z = 8 * (vol->px / 2) * (vol->py / 2);
+    } else if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) {
+        P.v.stride_y = 8 * (vol->px / 4);
+        P.v.stride_z = vol->px * vol->py;
     } else {
         P.v.stride_y = vol->px;
         P.v.stride_z = vol->px * vol->py;
@@ -178,6 +200,11 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "step %.6g mm is more than 120 voxels long", P.g.step);
     P.chunk = chunk;
     return GDRR_OK;
+}
+
+cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
+    return launch_project_exact(P, vol->vw, vol->layout, s);
 }
 
 }  // namespace
@@ -229,7 +256,9 @@ int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int lay
     if (!bytes) return fail(nullptr, GDRR_ERR_INVALID_ARG, "bytes is NULL");
     int rc = check_dims(nullptr, nx, ny, nz, n_materials, layout);
     if (rc) return rc;
-    *bytes = (size_t)padded(nx) * padded(ny) * padded(nz) * vector_width(n_materials) * sizeof(float);
+    int px, py, pz;
+    stored_dims(nx, ny, nz, layout, px, py, pz);
+    *bytes = (size_t)px * py * pz * element_bytes(n_materials, layout);
     return GDRR_OK;
 }
 
@@ -263,7 +292,7 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     IngestParams ip;
     ip.rho = rho_dev; ip.mat = material_dev; ip.vox = workspace_dev;
     ip.nx = nx; ip.ny = ny; ip.nz = nz;
-    ip.px = padded(nx); ip.py = padded(ny); ip.pz = padded(nz);
+    stored_dims(nx, ny, nz, layout, ip.px, ip.py, ip.pz);
     ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev;
     const int vw = vector_width(n_materials);
     e = launch_ingest(ip, vw, layout, s);
@@ -433,7 +462,7 @@ int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     P.signal = signal_dev; P.li = line_integrals_dev; P.ray_table = ray_table_dev;
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
-    cudaError_t e = launch_project(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
+    cudaError_t e = launch_project(P, vol, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "project kernel launch");
     ctx->launches += 1;
     return GDRR_OK;
@@ -475,7 +504,7 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
         Pb.g.proj_begin = proj_begin + done;
         Pb.g.proj_count = cnt;
         Pb.signal = stage; Pb.li = nullptr; Pb.ray_table = nullptr;
-        e = launch_project(Pb, vol->vw, vol->layout, s);
+        e = launch_project(Pb, vol, s);
         if (e != cudaSuccess) break;
         ctx->launches += 1;
         e = cudaEventRecord(ctx->ev_done[slot], s);

@@ -32,8 +32,8 @@ struct GeomParams {
 
 struct VolumeParams {
     const void* vox;                // device, layout below
-    int stride_y;                   // BRICK: 8 * bricks per row;      LINEAR: padded nx
-    int stride_z;                   // BRICK: 8 * bricks per slab;     LINEAR: padded nx * ny
+    int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: 8 * tiles per tile-row
+    int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab
 };
 
 struct ProjectParams {
@@ -55,14 +55,15 @@ struct IngestParams {
     const uint8_t* mat;
     void* vox;
     int nx, ny, nz;
-    int px, py, pz;                 // stored dims: N + 2 rounded up to even
+    int px, py, pz;                 // stored dims (voxels for BRICK / LINEAR, quads for PACKED_QUAD)
     int n_mat;
     int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
 };
 
 // Host-callable launchers (each returns the cudaGetLastError() of its launch).
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
-cudaError_t launch_project(const ProjectParams& p, int vw, int layout, cudaStream_t s);
+cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
+cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 

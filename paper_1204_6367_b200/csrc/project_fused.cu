@@ -1,20 +1,13 @@
-// Steps a1-a7 fused: ray setup, fixed-step tri-linear sampling of the
-// per-material density planes, and the energy sum.
+// Steps a1-a7 fused, EXACT layouts (GDRR_LAYOUT_BRICK / GDRR_LAYOUT_LINEAR):
+// ray setup, fixed-step tri-linear sampling of the per-material density planes,
+// and the energy sum.
 //
-// One thread per detector pixel.  A warp owns 8 (u) x 4 (v) adjacent pixels, so
-// at every step its 32 rays sit inside a few neighbouring 2x2x2 bricks and a
-// warp-wide corner load touches few 128-byte lines for every gantry angle.
-// The volume stores, per voxel, VW floats (one per material: rho at the voxel's
-// material, 0 elsewhere), so one vector load per corner serves all materials
-// and the 8 tri-linear weights are shared by them.
-//
-// Positions: every `chunk` samples the ray position is re-based in fp64 and
-// split into an integer cell and a 23-bit fixed-point fraction; inside a chunk
-// the position advances by integer adds, the cell is an arithmetic shift and
-// the weights come from OR-ing the fraction into the mantissa of a float in
-// [1, 2).  No float->int conversions in the loop; position error <= 2^-18 voxel.
-#include "gdrr_internal.h"
-#include "ray_setup.cuh"
+// One thread per detector pixel.  The volume stores, per voxel, VW floats (one
+// per material: rho at the voxel's material, 0 elsewhere), so one vector load
+// per corner serves all materials and the 8 tri-linear weights are shared by
+// them.  rho is kept bit-exact.  This is the reference layout of the library;
+// the packed-quad layout (project_packed.cu) is the fast one.
+#include "project_common.cuh"
 
 namespace gdrr {
 
@@ -55,37 +48,24 @@ template <int VW, int LAYOUT>
 __global__ void __launch_bounds__(kThreads)
 gdrr_project_kernel(const ProjectParams P) {
     using V = typename Vox<VW>::T;
-    extern __shared__ float4 smem_f4[];
-    float4* s_mu = smem_f4;                                   // [n_energy]
-    float2* s_src = reinterpret_cast<float2*>(s_mu + P.n_energy);  // [n_energy]
-    for (int e = threadIdx.x; e < P.n_energy; e += kThreads) {
-        s_mu[e] = P.mu_tab[e];
-        s_src[e] = P.src_tab[e];
-    }
-    __syncthreads();
+    float4* s_mu;
+    float2* s_src;
+    load_tables(P, s_mu, s_src);
 
-    // thread -> pixel: warp w covers an 8 x 4 block of the CTA's 16 x 16 tile
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int i = blockIdx.x * kTileU + (warp & 1) * 8 + (lane & 7);
-    const int j = blockIdx.y * kTileV + (warp >> 1) * 4 + (lane >> 3);
+    int i, j;
+    thread_pixel(i, j);
     const int pl = blockIdx.z;                                 // projection inside this call
     if (i >= P.g.nu || j >= P.g.nv) return;
 
     // ---- a1: ray setup (fp64) ------------------------------------------------
     Ray r;
     ray_setup(P.g, P.g.proj_begin + pl, i, j, r);
-    const size_t pix = ((size_t)pl * P.g.nv + j) * P.g.nu + i;
     if (P.ray_table) {
+        const size_t pix = ((size_t)pl * P.g.nv + j) * P.g.nu + i;
         reinterpret_cast<int2*>(P.ray_table)[pix] = make_int2(r.j0, r.n);
     }
-
-    // padded index coordinate of the point at parameter t:  q_a(t) = gs_a + t * (dir_a / d_a)
     double gs[3], dg[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        gs[a] = (r.S[a] - P.g.c[a]) / P.g.d[a] + P.g.ofs[a];
-        dg[a] = P.g.step * r.dir[a] / P.g.d[a];
-    }
+    index_line(P.g, r, gs, dg);
     const int dqx = __double2int_rn(dg[0] * 8388608.0);
     const int dqy = __double2int_rn(dg[1] * 8388608.0);
     const int dqz = __double2int_rn(dg[2] * 8388608.0);
@@ -100,16 +80,8 @@ gdrr_project_kernel(const ProjectParams P) {
     for (int m = 0; m < VW; ++m) acc[m] = 0.f;
 
     for (int kc = 0; kc < r.n; kc += P.chunk) {
-        // re-base: position of sample j0 + kc in fp64, split into cell + fraction
-        const double tk = (double)(r.j0 + kc) + 0.5;
-        const double bx = fma(tk, dg[0], gs[0]);
-        const double by = fma(tk, dg[1], gs[1]);
-        const double bz = fma(tk, dg[2], gs[2]);
-        const double fx = floor(bx), fy = floor(by), fz = floor(bz);
-        const int cbx = (int)fx, cby = (int)fy, cbz = (int)fz;
-        int qx = (int)((bx - fx) * 8388608.0);
-        int qy = (int)((by - fy) * 8388608.0);
-        int qz = (int)((bz - fz) * 8388608.0);
+        const ChunkBase b = chunk_base(gs, dg, r.j0 + kc);
+        int qx = b.qx, qy = b.qy, qz = b.qz;
         const int cnt = min(P.chunk, r.n - kc);
 
         float part[VW];
@@ -118,9 +90,9 @@ gdrr_project_kernel(const ProjectParams P) {
 
 #pragma unroll 2
         for (int s = 0; s < cnt; ++s) {
-            const int ix = cbx + (qx >> kFracBits);
-            const int iy = cby + (qy >> kFracBits);
-            const int iz = cbz + (qz >> kFracBits);
+            const int ix = b.cx + (qx >> kFracBits);
+            const int iy = b.cy + (qy >> kFracBits);
+            const int iz = b.cz + (qz >> kFracBits);
             const float Fx = __int_as_float((qx & 0x7FFFFF) | 0x3F800000);   // 1 + frac
             const float Fy = __int_as_float((qy & 0x7FFFFF) | 0x3F800000);
             const float Fz = __int_as_float((qz & 0x7FFFFF) | 0x3F800000);
@@ -160,45 +132,15 @@ gdrr_project_kernel(const ProjectParams P) {
         for (int m = 0; m < VW; ++m) acc[m] += part[m];
     }
 
-    // ---- a5: scale by dl ----------------------------------------------------------
-    float li[VW];
-#pragma unroll
-    for (int m = 0; m < VW; ++m) li[m] = (float)((double)acc[m] * P.g.step);
-    if (P.li) {
-        const size_t plane = (size_t)P.g.nv * P.g.nu;
-        float* o = P.li + (size_t)pl * P.n_mat * plane + (size_t)j * P.g.nu + i;
-#pragma unroll
-        for (int m = 0; m < VW; ++m)
-            if (m < P.n_mat) o[m * plane] = li[m];
-    }
-
-    // ---- a6: energy sum, tables in shared memory, exp as ex2 of pre-scaled args ---
-    const float tb = P.bt_thick ? P.bt_thick[i] : 0.f;
-    float sig = 0.f;
-    for (int e = 0; e < P.n_energy; ++e) {
-        const float4 mu = s_mu[e];
-        const float2 sc = s_src[e];
-        float tau = sc.y * tb;
-        tau = fmaf(mu.x, li[0], tau);
-        if (VW > 1) tau = fmaf(mu.y, li[VW > 1 ? 1 : 0], tau);
-        if (VW > 2) {
-            tau = fmaf(mu.z, li[VW > 2 ? 2 : 0], tau);
-            tau = fmaf(mu.w, li[VW > 2 ? 3 : 0], tau);
-        }
-        sig = fmaf(sc.x, exp2f(-tau), sig);
-    }
-    if (P.fluence) sig *= P.fluence[(size_t)j * P.g.nu + i];
-    // ---- a7 ------------------------------------------------------------------------
-    P.signal[pix] = sig;
+    finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
 }
 
 // Ray setup alone: the integer ray table and/or the sample count sum(n).
 __global__ void __launch_bounds__(kThreads)
 gdrr_ray_setup_kernel(const GeomParams g, int32_t* __restrict__ ray_table,
                       unsigned long long* __restrict__ n_samples) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int i = blockIdx.x * kTileU + (warp & 1) * 8 + (lane & 7);
-    const int j = blockIdx.y * kTileV + (warp >> 1) * 4 + (lane >> 3);
+    int i, j;
+    thread_pixel(i, j);
     const int pl = blockIdx.z;
     int n = 0;
     if (i < g.nu && j < g.nv) {
@@ -212,7 +154,7 @@ gdrr_ray_setup_kernel(const GeomParams g, int32_t* __restrict__ ray_table,
     }
     if (n_samples) {
         unsigned int tot = __reduce_add_sync(0xffffffffu, (unsigned int)n);
-        if (lane == 0 && tot) atomicAdd(n_samples, (unsigned long long)tot);
+        if ((threadIdx.x & 31) == 0 && tot) atomicAdd(n_samples, (unsigned long long)tot);
     }
 }
 
@@ -224,7 +166,7 @@ static cudaError_t launch_project_t(const ProjectParams& p, cudaStream_t s) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_project(const ProjectParams& p, int vw, int layout, cudaStream_t s) {
+cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s) {
     if (layout == 0) {
         if (vw == 1) return launch_project_t<1, 0>(p, s);
         if (vw == 2) return launch_project_t<2, 0>(p, s);

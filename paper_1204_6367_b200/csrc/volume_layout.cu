@@ -62,6 +62,39 @@ gdrr_ingest_kernel(const IngestParams P) {
     reinterpret_cast<V*>(P.vox)[o] = one_hot<VW>(rho, m);
 }
 
+// PACKED_QUAD (project_packed.cu): element (ex, ey, ez) = the four words of stored
+// voxels (ex, ey), (ex+1, ey), (ex, ey+1), (ex+1, ey+1) of slab ez; a word is rho
+// rounded to a 22-bit mantissa with the material index in the two freed bits
+// (n_mat > 1).  Slabs linear; inside a slab 4 (x) x 2 (y) tiles of 8 elements.
+__global__ void __launch_bounds__(256)
+gdrr_ingest_packed_kernel(const IngestParams P) {
+    const size_t total = (size_t)P.px * P.py * P.pz;
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= total) return;
+    const int e = (int)(o & 7);
+    size_t t = o >> 3;
+    const int ntx = P.px >> 2, nty = P.py >> 1;
+    const int tx = (int)(t % ntx);
+    t /= ntx;
+    const int ty = (int)(t % nty);
+    const int ez = (int)(t / nty);
+    const int ex = 4 * tx + (e & 3), ey = 2 * ty + (e >> 2);
+    const int iz = min(max(ez - 1, 0), P.nz - 1);
+    unsigned w[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int ix = min(max(ex + (k & 1) - 1, 0), P.nx - 1);
+        const int iy = min(max(ey + (k >> 1) - 1, 0), P.ny - 1);
+        const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
+        unsigned bits = __float_as_uint(P.rho[src]);
+        const unsigned m = P.mat[src];
+        if ((int)m >= P.n_mat) *P.bad_flag = 1;
+        if (P.n_mat > 1) bits = ((bits + 2u) & ~3u) | (m & 3u);
+        w[k] = bits;
+    }
+    reinterpret_cast<uint4*>(P.vox)[o] = make_uint4(w[0], w[1], w[2], w[3]);
+}
+
 template <int VW, int LAYOUT>
 static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
     const size_t total = (size_t)p.px * p.py * p.pz;
@@ -71,6 +104,11 @@ static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
 }
 
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s) {
+    if (layout == 2) {
+        const size_t total = (size_t)p.px * p.py * p.pz;
+        gdrr_ingest_packed_kernel<<<(unsigned int)((total + 255) / 256), 256, 0, s>>>(p);
+        return cudaGetLastError();
+    }
     if (layout == 0) {
         if (vw == 1) return launch_ingest_t<1, 0>(p, s);
         if (vw == 2) return launch_ingest_t<2, 0>(p, s);

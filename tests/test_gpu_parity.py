@@ -30,7 +30,7 @@ def gdrr():
     return g
 
 
-LAYOUTS = [0, 1]
+LAYOUTS = [0, 1, 2]
 
 
 # ---------------------------------------------------------------- C0 .. C2, full images
