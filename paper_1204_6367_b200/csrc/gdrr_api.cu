@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -37,6 +38,7 @@ struct gdrr_context {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
+    int variant = 0;            // kernel variant under exploration (GDRR_VARIANT), 0 = default
 };
 
 struct gdrr_volume {
@@ -199,11 +201,13 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     if (chunk < 1)
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "step %.6g mm is more than 120 voxels long", P.g.step);
     P.chunk = chunk;
+    P.frac_mask = 0x007FFFFFu;
+    P.one_bits = 0x3F800000u;
     return GDRR_OK;
 }
 
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
-    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, vol->ctx->variant, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);
 }
 
@@ -224,6 +228,7 @@ int gdrr_create_context(int cuda_device, gdrr_context** out) {
     gdrr_context* ctx = new (std::nothrow) gdrr_context;
     if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "out of host memory");
     ctx->device = cuda_device;
+    if (const char* v = std::getenv("GDRR_VARIANT")) ctx->variant = std::atoi(v);
     DeviceGuard guard(cuda_device);
     if (guard.status != cudaSuccess) { delete ctx; return cuda_fail(nullptr, guard.status, "cudaSetDevice"); }
     e = cudaMalloc(&ctx->flag_dev, sizeof(int));

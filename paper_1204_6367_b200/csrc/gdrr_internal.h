@@ -45,6 +45,7 @@ struct ProjectParams {
     const float* fluence;           // [nv][nu] or nullptr
     int n_energy, n_mat;
     int chunk;                      // <= kMaxChunk
+    unsigned frac_mask, one_bits;   // 0x007FFFFF, 0x3F800000: kept in registers by the samplers
     float* signal;                  // [proj_count][nv][nu]
     float* li;                      // [proj_count][n_mat][nv][nu] or nullptr
     int32_t* ray_table;             // [proj_count][nv][nu][2] or nullptr
@@ -63,7 +64,7 @@ struct IngestParams {
 // Host-callable launchers (each returns the cudaGetLastError() of its launch).
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
-cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
+cudaError_t launch_project_packed(const ProjectParams& p, int vw, int variant, cudaStream_t s);
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 

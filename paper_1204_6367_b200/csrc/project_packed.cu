@@ -33,8 +33,21 @@ __device__ __forceinline__ void add_routed(float (&part)[VW], int m, float v) {
 
 __device__ __forceinline__ float lerp(float a, float b, float t) { return fmaf(t, b - a, a); }
 
-template <int VW>
-__global__ void __launch_bounds__(kThreads)
+// (q & mask) | one in a single LOP3; mask and one arrive as kernel parameters so
+// that they live in registers instead of being split into two immediate ops.
+__device__ __forceinline__ float frac_float(int q, unsigned mask, unsigned one) {
+    unsigned o;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(o) : "r"(q), "r"(mask), "r"(one));
+    return __uint_as_float(o) - 1.f;
+}
+
+// element index: slabs linear, 4 (x) x 2 (y) tiles of 8 quads = 128 B inside a slab
+__device__ __forceinline__ int quad_index(int ix, int iy, int iz, int sy, int sz) {
+    return iz * sz + (iy >> 1) * sy + ((iy & 1) << 2) + ix + (ix & ~3);
+}
+
+template <int VW, int MINB, int UNROLL>
+__global__ void __launch_bounds__(kThreads, MINB)
 gdrr_project_packed_kernel(const ProjectParams P) {
     float4* s_mu;
     float2* s_src;
@@ -58,13 +71,17 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     const int dqy = __double2int_rn(dg[1] * 8388608.0);
     const int dqz = __double2int_rn(dg[2] * 8388608.0);
 
-    const uint4* __restrict__ vol = reinterpret_cast<const uint4*>(P.v.vox);
     const int sy = P.v.stride_y, sz = P.v.stride_z;
+    const uint4* __restrict__ vol0 = reinterpret_cast<const uint4*>(P.v.vox);   // slab iz
+    const uint4* __restrict__ vol1 = vol0 + sz;                                  // slab iz + 1
+    const unsigned fmask = P.frac_mask, fone = P.one_bits;
 
     // ---- a2-a4: sampling -------------------------------------------------------
     float acc[VW];
 #pragma unroll
     for (int m = 0; m < VW; ++m) acc[m] = 0.f;
+    unsigned curm = 0;         // material of the running sum of pure cells
+    float cur = 0.f;
 
     for (int kc = 0; kc < r.n; kc += P.chunk) {
         const ChunkBase b = chunk_base(gs, dg, r.j0 + kc);
@@ -74,44 +91,43 @@ gdrr_project_packed_kernel(const ProjectParams P) {
         float part[VW];
 #pragma unroll
         for (int m = 0; m < VW; ++m) part[m] = 0.f;
-        int curm = 0;          // material of the running sum of pure cells
-        float cur = 0.f;
 
-#pragma unroll 2
+        // software pipeline: the two loads of sample s + 1 are in flight while sample s is blended
+        int idx = quad_index(b.cx, b.cy, b.cz, sy, sz);
+        uint4 a = __ldg(vol0 + idx);            // slab iz:     (x0y0, x1y0, x0y1, x1y1)
+        uint4 c = __ldg(vol1 + idx);            // slab iz + 1
+
+#pragma unroll UNROLL
         for (int s = 0; s < cnt; ++s) {
-            const int ix = b.cx + (qx >> kFracBits);
-            const int iy = b.cy + (qy >> kFracBits);
-            const int iz = b.cz + (qz >> kFracBits);
-            const float fx = __int_as_float((qx & 0x7FFFFF) | 0x3F800000) - 1.f;
-            const float fy = __int_as_float((qy & 0x7FFFFF) | 0x3F800000) - 1.f;
-            const float fz = __int_as_float((qz & 0x7FFFFF) | 0x3F800000) - 1.f;
-            // element index: slabs linear, 4 (x) x 2 (y) tiles of 8 quads = 128 B inside a slab
-            const int idx = iz * sz + (iy >> 1) * sy + ((iy & 1) << 2) + ix + (ix & ~3);
-            const uint4 a = __ldg(vol + idx);           // slab iz:     (x0y0, x1y0, x0y1, x1y1)
-            const uint4 c = __ldg(vol + idx + sz);      // slab iz + 1
-
-            bool pure = true;
-            if (VW > 1) {
-                const unsigned d = (a.x ^ a.y) | (a.x ^ a.z) | (a.x ^ a.w) | (a.x ^ c.x) | (a.x ^ c.y) |
-                                   (a.x ^ c.z) | (a.x ^ c.w);
-                pure = (d & 3u) == 0u;
+            const float fx = frac_float(qx, fmask, fone);
+            const float fy = frac_float(qy, fmask, fone);
+            const float fz = frac_float(qz, fmask, fone);
+            qx += dqx;
+            qy += dqy;
+            qz += dqz;
+            uint4 an = a, cn = c;
+            if (s + 1 < cnt) {
+                idx = quad_index(b.cx + (qx >> kFracBits), b.cy + (qy >> kFracBits),
+                                 b.cz + (qz >> kFracBits), sy, sz);
+                an = __ldg(vol0 + idx);
+                cn = __ldg(vol1 + idx);
             }
-            if (pure) {
+
+            bool fast = true;
+            if (VW > 1) {
+                // all 8 corners of the current material?  (two lowest bits of every word)
+                const unsigned d = (a.x ^ a.y) | (a.x ^ a.z) | (a.x ^ a.w) | (a.x ^ c.x) | (a.x ^ c.y) |
+                                   (a.x ^ c.z) | (a.x ^ c.w) | (a.x ^ curm);
+                fast = (d & 3u) == 0u;
+            }
+            if (fast) {
                 const float v0 = lerp(lerp(__uint_as_float(a.x), __uint_as_float(a.y), fx),
                                       lerp(__uint_as_float(a.z), __uint_as_float(a.w), fx), fy);
                 const float v1 = lerp(lerp(__uint_as_float(c.x), __uint_as_float(c.y), fx),
                                       lerp(__uint_as_float(c.z), __uint_as_float(c.w), fx), fy);
-                const float v = lerp(v0, v1, fz);
-                if (VW > 1) {
-                    const int m = (int)(a.x & 3u);
-                    if (m != curm) {
-                        add_routed<VW>(part, curm, cur);
-                        cur = 0.f;
-                        curm = m;
-                    }
-                }
-                cur += v;
+                cur += lerp(v0, v1, fz);
             } else {
+                // mixed cell, or a pure cell of another material: route every weighted corner
                 const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
                 const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
                 add_routed<VW>(part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
@@ -122,12 +138,19 @@ gdrr_project_packed_kernel(const ProjectParams P) {
                 add_routed<VW>(part, (int)(c.y & 3u), fx * w01 * __uint_as_float(c.y));
                 add_routed<VW>(part, (int)(c.z & 3u), gx * w11 * __uint_as_float(c.z));
                 add_routed<VW>(part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
+                // the running sum follows the material the ray is now in
+                const unsigned m = c.w & 3u;
+                if (m != curm) {
+                    add_routed<VW>(part, (int)curm, cur);
+                    cur = 0.f;
+                    curm = m;
+                }
             }
-            qx += dqx;
-            qy += dqy;
-            qz += dqz;
+            a = an;
+            c = cn;
         }
-        add_routed<VW>(part, curm, cur);
+        add_routed<VW>(part, (int)curm, cur);
+        cur = 0.f;
 #pragma unroll
         for (int m = 0; m < VW; ++m) acc[m] += part[m];
     }
@@ -135,13 +158,28 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
 }
 
-cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s) {
+template <int VW, int MINB, int UNROLL>
+static cudaError_t launch_packed_t(const ProjectParams& p, cudaStream_t s) {
     dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
     const size_t smem = (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
-    if (vw == 1) gdrr_project_packed_kernel<1><<<grid, kThreads, smem, s>>>(p);
-    else if (vw == 2) gdrr_project_packed_kernel<2><<<grid, kThreads, smem, s>>>(p);
-    else gdrr_project_packed_kernel<4><<<grid, kThreads, smem, s>>>(p);
+    gdrr_project_packed_kernel<VW, MINB, UNROLL><<<grid, kThreads, smem, s>>>(p);
     return cudaGetLastError();
+}
+
+cudaError_t launch_project_packed(const ProjectParams& p, int vw, int variant, cudaStream_t s) {
+    if (vw == 1) return launch_packed_t<1, 4, 2>(p, s);
+    if (vw == 2) return launch_packed_t<2, 4, 2>(p, s);
+    switch (variant) {
+        case 1: return launch_packed_t<4, 3, 2>(p, s);
+        case 2: return launch_packed_t<4, 5, 2>(p, s);
+        case 3: return launch_packed_t<4, 6, 2>(p, s);
+        case 4: return launch_packed_t<4, 4, 1>(p, s);
+        case 5: return launch_packed_t<4, 5, 1>(p, s);
+        case 6: return launch_packed_t<4, 6, 1>(p, s);
+        case 7: return launch_packed_t<4, 4, 4>(p, s);
+        case 8: return launch_packed_t<4, 3, 4>(p, s);
+        default: return launch_packed_t<4, 4, 2>(p, s);
+    }
 }
 
 }  // namespace gdrr
