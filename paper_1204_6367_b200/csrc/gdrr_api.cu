@@ -2,6 +2,7 @@
 // small context-owned device tables, and kernel launches.  No arithmetic of the
 // method happens here except what the header says is done on the host: cos/sin
 // of the gantry angles (given to the kernels as data) and table pre-scaling.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -47,6 +48,7 @@ struct gdrr_volume {
     int nx, ny, nz, px, py, pz;
     double d[3], c[3];
     int n_mat, vw, layout;
+    int sy, sz, packed_lay;     // PACKED_QUAD: element strides and order
 };
 
 static thread_local std::string g_create_err;
@@ -98,6 +100,28 @@ void stored_dims(int nx, int ny, int nz, int layout, int& px, int& py, int& pz) 
     }
 }
 
+// PACKED_QUAD element strides.  Order 0: slabs linear, 4 x 2 tiles of 8 elements in a slab
+// (px, py already rounded to the tile).  Order 1: linear with row stride = 3 and slab stride
+// = 4 (mod 8), so that neighbouring elements fall in different 16-byte bank groups of the L1
+// data RAM in every direction (project_packed.cu).
+void packed_strides(int px, int py, int lay, int& sy, int& sz) {
+    if (lay == 0) {
+        sy = 8 * (px / 4);
+        sz = px * py;
+    } else {
+        sy = px + ((3 - px % 8) + 8) % 8;
+        const long long s0 = (long long)sy * py;
+        sz = (int)(s0 + ((4 - s0 % 8) + 8) % 8);
+    }
+}
+
+size_t packed_elements(int nx, int ny, int nz, int lay) {
+    int px, py, pz, sy, sz;
+    stored_dims(nx, ny, nz, GDRR_LAYOUT_PACKED_QUAD, px, py, pz);
+    packed_strides(px, py, lay, sy, sz);
+    return (size_t)sz * pz;
+}
+
 size_t element_bytes(int n_mat, int layout) {
     return layout == GDRR_LAYOUT_PACKED_QUAD ? 16 : vector_width(n_mat) * sizeof(float);
 }
@@ -121,7 +145,9 @@ int check_dims(gdrr_context* ctx, int nx, int ny, int nz, int n_materials, int l
         return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown layout %d", layout);
     int px, py, pz;
     stored_dims(nx, ny, nz, layout, px, py, pz);
-    const double total = (double)px * py * pz;
+    double total = (double)px * py * pz;
+    if (layout == GDRR_LAYOUT_PACKED_QUAD)
+        total = (double)std::max(packed_elements(nx, ny, nz, 0), packed_elements(nx, ny, nz, 1)) + px * (double)py;
     if (total >= 2147483648.0)
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "padded volume has %.0f voxels; the sampler indexes with int32", total);
     return GDRR_OK;
@@ -181,12 +207,13 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
         P.v.stride_y = 8 * (vol->px / 2);
         P.v.stride_z = 8 * (vol->px / 2) * (vol->py / 2);
     } else if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) {
-        P.v.stride_y = 8 * (vol->px / 4);
-        P.v.stride_z = vol->px * vol->py;
+        P.v.stride_y = vol->sy;
+        P.v.stride_z = vol->sz;
     } else {
         P.v.stride_y = vol->px;
         P.v.stride_z = vol->px * vol->py;
     }
+    P.v.packed_lay = vol->packed_lay;
     P.mu_tab = ctx->mu_dev;
     P.src_tab = ctx->src_dev;
     P.bt_thick = ctx->bt_dev;
@@ -264,6 +291,8 @@ int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int lay
     int px, py, pz;
     stored_dims(nx, ny, nz, layout, px, py, pz);
     *bytes = (size_t)px * py * pz * element_bytes(n_materials, layout);
+    if (layout == GDRR_LAYOUT_PACKED_QUAD)      // either element order fits
+        *bytes = 16 * std::max(packed_elements(nx, ny, nz, 0), packed_elements(nx, ny, nz, 1));
     return GDRR_OK;
 }
 
@@ -299,6 +328,9 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     ip.nx = nx; ip.ny = ny; ip.nz = nz;
     stored_dims(nx, ny, nz, layout, ip.px, ip.py, ip.pz);
     ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev;
+    ip.sy = ip.sz = 0;
+    ip.packed_lay = (ctx->variant & 1) ? 0 : 1;
+    if (layout == GDRR_LAYOUT_PACKED_QUAD) packed_strides(ip.px, ip.py, ip.packed_lay, ip.sy, ip.sz);
     const int vw = vector_width(n_materials);
     e = launch_ingest(ip, vw, layout, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel launch");
@@ -316,6 +348,7 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     v->d[0] = dx_mm; v->d[1] = dy_mm; v->d[2] = dz_mm;
     for (int a = 0; a < 3; ++a) v->c[a] = centre_mm ? centre_mm[a] : 0.0;
     v->n_mat = n_materials; v->vw = vw; v->layout = layout;
+    v->sy = ip.sy; v->sz = ip.sz; v->packed_lay = ip.packed_lay;
     *out = v;
     return GDRR_OK;
 }

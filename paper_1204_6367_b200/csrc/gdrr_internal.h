@@ -34,6 +34,7 @@ struct VolumeParams {
     const void* vox;                // device, layout below
     int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: 8 * tiles per tile-row
     int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab
+    int packed_lay;                 // PACKED_QUAD element order: 0 = 4 x 2 tiles in a slab, 1 = linear with skewed strides
 };
 
 struct ProjectParams {
@@ -57,6 +58,7 @@ struct IngestParams {
     void* vox;
     int nx, ny, nz;
     int px, py, pz;                 // stored dims (voxels for BRICK / LINEAR, quads for PACKED_QUAD)
+    int sy, sz, packed_lay;         // PACKED_QUAD: element strides and order (VolumeParams)
     int n_mat;
     int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
 };

@@ -1,25 +1,32 @@
 // Steps a1-a7 fused, PACKED-QUAD layout (GDRR_LAYOUT_PACKED_QUAD): the fast path.
 //
-// Why this layout.  ncu on the one-hot float4 kernel (profiles/r01_v1_onehot.md):
-// l1tex data-pipe wavefronts at 95% of peak, 10.2 wavefronts per 16-byte
-// warp-wide load and 8 such loads per sample -- the kernel is bound by L1
-// wavefronts, not by bytes, DRAM or issue slots.  So the lever is wavefronts
-// per sample.  Here a voxel is ONE 32-bit word: fp32 rho whose two lowest
-// mantissa bits carry the material index (n_materials > 1), and element
-// (ix, iy, iz) of the device volume is the 2x2 quad of words
+// Layout.  A voxel is ONE 32-bit word: fp32 rho whose three lowest mantissa
+// bits carry tags (n_materials > 1): bits 0-1 the material index, bit 2 (first
+// word of an element only) "all 8 corners of this cell have this material".
+// Element (ix, iy, iz) of the device volume is the 2x2 quad of words
 // {(ix,iy), (ix+1,iy), (ix,iy+1), (ix+1,iy+1)} of slab iz, stored for EVERY
-// (ix, iy) (quads overlap, 16 B per voxel like the float4 layout).  A sample
-// then needs two 16-byte loads (slabs iz and iz+1) instead of eight.
+// (ix, iy) (quads overlap, 16 B per voxel).  A sample needs two 16-byte loads
+// (slabs iz and iz+1).
 //
-// Material routing.  In a segmented volume almost every cell is pure (all 8
-// corners of one material: 98.8% of C3's cells), so the common path is one
-// scalar tri-linear blend added to a running sum that is routed to its
-// material only when the material changes; cells with mixed corners take a
-// slower branch that routes each weighted corner.  Both give the same value.
+// What bounds the gather (profiles/r01_l1_model.md, measured on B200): a 16-byte
+// warp-wide load is served in 4 phases of 8 lanes; inside a phase, distinct
+// elements whose index is equal mod 8 (same 16-byte bank group of the L1 data
+// RAM) serialise, whatever line they are in; the tag stage takes 4 lines per
+// cycle.  So (1) the lanes of a warp must sample the SAME interval index k at
+// the same time (intervals are laid from the source, so equal k is a sphere
+// around the source and the warp's footprint stays a compact 2-D patch; starting
+// every ray at its own j0 spreads the warp over up to 8 steps of depth), and
+// (2) neighbouring elements must differ mod 8 in every direction: elements are
+// stored linearly with the row stride = 3 and the slab stride = 4 (mod 8).
 //
-// The words are used as floats as they are (the material bits are part of the
-// stored value: |stored - rho| <= 5 ulp, 3e-7 relative; DESIGN.md "Packed
-// words"); the library is compiled with -ftz=true so that rho = 0 tagged with a
+// Material routing.  In a segmented volume almost every cell is pure (98.8% of
+// C3's cells), so the common path is one scalar tri-linear blend added to a
+// running sum that is routed to its material only when the material changes;
+// cells with mixed corners take a slower branch that routes each weighted
+// corner.  Both give the same value.
+//
+// The words are used as floats as they are (|stored - rho| <= 11 ulp, DESIGN.md
+// Q24); the library is compiled with -ftz=true so that rho = 0 tagged with a
 // material (a denormal bit pattern) contributes exactly 0.
 #include "project_common.cuh"
 
@@ -41,12 +48,71 @@ __device__ __forceinline__ float frac_float(int q, unsigned mask, unsigned one) 
     return __uint_as_float(o) - 1.f;
 }
 
-// element index: slabs linear, 4 (x) x 2 (y) tiles of 8 quads = 128 B inside a slab
-__device__ __forceinline__ int quad_index(int ix, int iy, int iz, int sy, int sz) {
-    return iz * sz + (iy >> 1) * sy + ((iy & 1) << 2) + ix + (ix & ~3);
+// thread -> pixel.  LMAP 0: a warp is 8 (u) x 4 (v) pixels, a load phase (8 lanes)
+// one row of 8; LMAP 1: a warp is 4 (u) x 8 (v), a phase 4 x 2 pixels.
+template <int LMAP>
+__device__ __forceinline__ void thread_pixel_map(int& i, int& j) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (LMAP == 0) {
+        i = blockIdx.x * kTileU + (warp & 1) * 8 + (lane & 7);
+        j = blockIdx.y * kTileV + (warp >> 1) * 4 + (lane >> 3);
+    } else {
+        i = blockIdx.x * kTileU + (warp & 3) * 4 + (lane & 3);
+        j = blockIdx.y * kTileV + (warp >> 2) * 8 + (lane >> 2);
+    }
 }
 
-template <int VW, int MINB, int UNROLL>
+// Element index of cell (cx, cy, cz).  LAY 0: 4 (x) x 2 (y) tiles of 8 elements
+// inside a slab; LAY 1: linear, skewed strides.
+template <int LAY>
+__device__ __forceinline__ int elem_index(int cx, int cy, int cz, int sy, int sz) {
+    if (LAY == 0) return cz * sz + (cy >> 1) * sy + ((cy & 1) << 2) + cx + (cx & ~3);
+    return cz * sz + cy * sy + cx;
+}
+
+// One sample: blend the 8 corners (a = slab iz, c = slab iz + 1) with the
+// fractions (fx, fy, fz) and add to the running sums.
+template <int VW>
+__device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, float fx, float fy, float fz,
+                                             float& cur, unsigned& curm4, float (&part)[VW]) {
+    bool fast = true;
+    if (VW > 1) fast = (a.x & 7u) == curm4;        // pure cell of the running material
+    if (fast) {
+        const float v0 = lerp(lerp(__uint_as_float(a.x), __uint_as_float(a.y), fx),
+                              lerp(__uint_as_float(a.z), __uint_as_float(a.w), fx), fy);
+        const float v1 = lerp(lerp(__uint_as_float(c.x), __uint_as_float(c.y), fx),
+                              lerp(__uint_as_float(c.z), __uint_as_float(c.w), fx), fy);
+        cur += lerp(v0, v1, fz);
+    } else {
+        // mixed cell, or a pure cell of another material: route every weighted corner
+        const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
+        const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
+        add_routed<VW>(part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
+        add_routed<VW>(part, (int)(a.y & 3u), fx * w00 * __uint_as_float(a.y));
+        add_routed<VW>(part, (int)(a.z & 3u), gx * w10 * __uint_as_float(a.z));
+        add_routed<VW>(part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
+        add_routed<VW>(part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
+        add_routed<VW>(part, (int)(c.y & 3u), fx * w01 * __uint_as_float(c.y));
+        add_routed<VW>(part, (int)(c.z & 3u), gx * w11 * __uint_as_float(c.z));
+        add_routed<VW>(part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
+        // the running sum follows the material the ray is now in
+        const unsigned m4 = (c.w & 3u) | 4u;
+        if (m4 != curm4) {
+            add_routed<VW>(part, (int)(curm4 & 3u), cur);
+            cur = 0.f;
+            curm4 = m4;
+        }
+    }
+}
+
+template <int LAY>
+__device__ __forceinline__ int sample_index(const ChunkBase& b, int idx0, int qx, int qy, int qz, int sy, int sz) {
+    if (LAY == 0)
+        return elem_index<0>(b.cx + (qx >> kFracBits), b.cy + (qy >> kFracBits), b.cz + (qz >> kFracBits), sy, sz);
+    return idx0 + (qz >> kFracBits) * sz + (qy >> kFracBits) * sy + (qx >> kFracBits);
+}
+
+template <int VW, int LAY, int LMAP, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB)
 gdrr_project_packed_kernel(const ProjectParams P) {
     float4* s_mu;
@@ -54,14 +120,16 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     load_tables(P, s_mu, s_src);
 
     int i, j;
-    thread_pixel(i, j);
+    thread_pixel_map<LMAP>(i, j);
     const int pl = blockIdx.z;
-    if (i >= P.g.nu || j >= P.g.nv) return;
+    // lanes outside the detector stay in the warp (the loop below is warp-synchronous) with n = 0
+    const bool valid = i < P.g.nu && j < P.g.nv;
 
     // ---- a1: ray setup (fp64) ------------------------------------------------
     Ray r;
-    ray_setup(P.g, P.g.proj_begin + pl, i, j, r);
-    if (P.ray_table) {
+    ray_setup(P.g, P.g.proj_begin + pl, min(i, P.g.nu - 1), min(j, P.g.nv - 1), r);
+    if (!valid) r.n = 0;
+    if (valid && P.ray_table) {
         const size_t pix = ((size_t)pl * P.g.nv + j) * P.g.nu + i;
         reinterpret_cast<int2*>(P.ray_table)[pix] = make_int2(r.j0, r.n);
     }
@@ -76,110 +144,109 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     const uint4* __restrict__ vol1 = vol0 + sz;                                  // slab iz + 1
     const unsigned fmask = P.frac_mask, fone = P.one_bits;
 
+    // Interval indices k are counted from the source (reading Q9), so all lanes of the
+    // warp walk the same k: the warp's samples lie on a sphere around the source.
+    const int kmin = __reduce_min_sync(0xffffffffu, r.n > 0 ? r.j0 : 0x7fffffff);
+    const int kmax = __reduce_max_sync(0xffffffffu, r.n > 0 ? r.j0 + r.n : (int)0x80000000);
+    const unsigned un = (unsigned)r.n;
+    const int CH = P.chunk;
+
     // ---- a2-a4: sampling -------------------------------------------------------
     float acc[VW];
 #pragma unroll
     for (int m = 0; m < VW; ++m) acc[m] = 0.f;
-    unsigned curm = 0;         // material of the running sum of pure cells
+    unsigned curm4 = 4u;       // 4 | material of the running sum of pure cells
     float cur = 0.f;
 
-    for (int kc = 0; kc < r.n; kc += P.chunk) {
-        const ChunkBase b = chunk_base(gs, dg, r.j0 + kc);
+    for (int kc = (kmin / CH) * CH; kc < kmax; kc += CH) {
+        const int s0 = max(kmin - kc, 0);
+        const int cnt = min(kmax - kc, CH) - s0;
+        const ChunkBase b = chunk_base(gs, dg, kc + s0);
         int qx = b.qx, qy = b.qy, qz = b.qz;
-        const int cnt = min(P.chunk, r.n - kc);
+        const int idx0 = (LAY == 0) ? 0 : elem_index<1>(b.cx, b.cy, b.cz, sy, sz);
+        unsigned rel = (unsigned)(kc + s0 - r.j0);      // sample s of the chunk is this ray's iff rel + s < n
 
         float part[VW];
 #pragma unroll
         for (int m = 0; m < VW; ++m) part[m] = 0.f;
 
-        // software pipeline: the two loads of sample s + 1 are in flight while sample s is blended
-        int idx = quad_index(b.cx, b.cy, b.cz, sy, sz);
-        uint4 a = __ldg(vol0 + idx);            // slab iz:     (x0y0, x1y0, x0y1, x1y1)
-        uint4 c = __ldg(vol1 + idx);            // slab iz + 1
-
-#pragma unroll UNROLL
-        for (int s = 0; s < cnt; ++s) {
-            const float fx = frac_float(qx, fmask, fone);
-            const float fy = frac_float(qy, fmask, fone);
-            const float fz = frac_float(qz, fmask, fone);
-            qx += dqx;
-            qy += dqy;
-            qz += dqz;
-            uint4 an = a, cn = c;
-            if (s + 1 < cnt) {
-                idx = quad_index(b.cx + (qx >> kFracBits), b.cy + (qy >> kFracBits),
-                                 b.cz + (qz >> kFracBits), sy, sz);
-                an = __ldg(vol0 + idx);
-                cn = __ldg(vol1 + idx);
-            }
-
-            bool fast = true;
-            if (VW > 1) {
-                // all 8 corners of the current material?  (two lowest bits of every word)
-                const unsigned d = (a.x ^ a.y) | (a.x ^ a.z) | (a.x ^ a.w) | (a.x ^ c.x) | (a.x ^ c.y) |
-                                   (a.x ^ c.z) | (a.x ^ c.w) | (a.x ^ curm);
-                fast = (d & 3u) == 0u;
-            }
-            if (fast) {
-                const float v0 = lerp(lerp(__uint_as_float(a.x), __uint_as_float(a.y), fx),
-                                      lerp(__uint_as_float(a.z), __uint_as_float(a.w), fx), fy);
-                const float v1 = lerp(lerp(__uint_as_float(c.x), __uint_as_float(c.y), fx),
-                                      lerp(__uint_as_float(c.z), __uint_as_float(c.w), fx), fy);
-                cur += lerp(v0, v1, fz);
-            } else {
-                // mixed cell, or a pure cell of another material: route every weighted corner
-                const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
-                const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
-                add_routed<VW>(part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
-                add_routed<VW>(part, (int)(a.y & 3u), fx * w00 * __uint_as_float(a.y));
-                add_routed<VW>(part, (int)(a.z & 3u), gx * w10 * __uint_as_float(a.z));
-                add_routed<VW>(part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
-                add_routed<VW>(part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
-                add_routed<VW>(part, (int)(c.y & 3u), fx * w01 * __uint_as_float(c.y));
-                add_routed<VW>(part, (int)(c.z & 3u), gx * w11 * __uint_as_float(c.z));
-                add_routed<VW>(part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
-                // the running sum follows the material the ray is now in
-                const unsigned m = c.w & 3u;
-                if (m != curm) {
-                    add_routed<VW>(part, (int)curm, cur);
-                    cur = 0.f;
-                    curm = m;
-                }
-            }
-            a = an;
-            c = cn;
+        // two register buffers: the loads of sample s + 1 are in flight while sample s is blended
+        uint4 a0 = make_uint4(0, 0, 0, 0), c0 = a0, a1 = a0, c1 = a0;
+        bool act0 = rel < un;
+        if (act0) {
+            const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, sy, sz);
+            a0 = __ldg(vol0 + idx);
+            c0 = __ldg(vol1 + idx);
         }
-        add_routed<VW>(part, (int)curm, cur);
+        for (int s = 0; s < cnt; s += 2) {
+            float fx = frac_float(qx, fmask, fone);
+            float fy = frac_float(qy, fmask, fone);
+            float fz = frac_float(qz, fmask, fone);
+            qx += dqx; qy += dqy; qz += dqz;
+            const bool more = s + 1 < cnt;                       // warp-uniform
+            const bool act1 = more && (rel + 1u < un);
+            if (act1) {
+                const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, sy, sz);
+                a1 = __ldg(vol0 + idx);
+                c1 = __ldg(vol1 + idx);
+            }
+            if (act0) blend_sample<VW>(a0, c0, fx, fy, fz, cur, curm4, part);
+            if (more) {
+                fx = frac_float(qx, fmask, fone);
+                fy = frac_float(qy, fmask, fone);
+                fz = frac_float(qz, fmask, fone);
+                qx += dqx; qy += dqy; qz += dqz;
+                rel += 2u;
+                act0 = (s + 2 < cnt) && (rel < un);
+                if (act0) {
+                    const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, sy, sz);
+                    a0 = __ldg(vol0 + idx);
+                    c0 = __ldg(vol1 + idx);
+                }
+                if (act1) blend_sample<VW>(a1, c1, fx, fy, fz, cur, curm4, part);
+            }
+        }
+        add_routed<VW>(part, (int)(curm4 & 3u), cur);
         cur = 0.f;
 #pragma unroll
         for (int m = 0; m < VW; ++m) acc[m] += part[m];
     }
 
-    finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
+    if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
 }
 
-template <int VW, int MINB, int UNROLL>
+template <int VW, int LAY, int LMAP, int MINB>
 static cudaError_t launch_packed_t(const ProjectParams& p, cudaStream_t s) {
     dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
     const size_t smem = (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
-    gdrr_project_packed_kernel<VW, MINB, UNROLL><<<grid, kThreads, smem, s>>>(p);
+    gdrr_project_packed_kernel<VW, LAY, LMAP, MINB><<<grid, kThreads, smem, s>>>(p);
     return cudaGetLastError();
 }
 
-cudaError_t launch_project_packed(const ProjectParams& p, int vw, int variant, cudaStream_t s) {
-    if (vw == 1) return launch_packed_t<1, 4, 2>(p, s);
-    if (vw == 2) return launch_packed_t<2, 4, 2>(p, s);
-    switch (variant) {
-        case 1: return launch_packed_t<4, 3, 2>(p, s);
-        case 2: return launch_packed_t<4, 5, 2>(p, s);
-        case 3: return launch_packed_t<4, 6, 2>(p, s);
-        case 4: return launch_packed_t<4, 4, 1>(p, s);
-        case 5: return launch_packed_t<4, 5, 1>(p, s);
-        case 6: return launch_packed_t<4, 6, 1>(p, s);
-        case 7: return launch_packed_t<4, 4, 4>(p, s);
-        case 8: return launch_packed_t<4, 3, 4>(p, s);
-        default: return launch_packed_t<4, 4, 2>(p, s);
+template <int VW, int LAY>
+static cudaError_t launch_packed_l(const ProjectParams& p, int variant, cudaStream_t s) {
+    const int lmap = (variant >> 1) & 1, occ = (variant >> 2) & 3;
+    if (lmap == 0) {
+        if (occ == 1) return launch_packed_t<VW, LAY, 0, 3>(p, s);
+        if (occ == 2) return launch_packed_t<VW, LAY, 0, 5>(p, s);
+        return launch_packed_t<VW, LAY, 0, 4>(p, s);
     }
+    if (occ == 1) return launch_packed_t<VW, LAY, 1, 3>(p, s);
+    if (occ == 2) return launch_packed_t<VW, LAY, 1, 5>(p, s);
+    return launch_packed_t<VW, LAY, 1, 4>(p, s);
+}
+
+// variant: bit 1 = lane map, bits 2-3 = occupancy target; the element order (p.v.packed_lay)
+// is a property of the ingested volume.
+cudaError_t launch_project_packed(const ProjectParams& p, int vw, int variant, cudaStream_t s) {
+    if (p.v.packed_lay == 0) {
+        if (vw == 1) return launch_packed_l<1, 0>(p, variant, s);
+        if (vw == 2) return launch_packed_l<2, 0>(p, variant, s);
+        return launch_packed_l<4, 0>(p, variant, s);
+    }
+    if (vw == 1) return launch_packed_l<1, 1>(p, variant, s);
+    if (vw == 2) return launch_packed_l<2, 1>(p, variant, s);
+    return launch_packed_l<4, 1>(p, variant, s);
 }
 
 }  // namespace gdrr

@@ -63,36 +63,56 @@ gdrr_ingest_kernel(const IngestParams P) {
 }
 
 // PACKED_QUAD (project_packed.cu): element (ex, ey, ez) = the four words of stored
-// voxels (ex, ey), (ex+1, ey), (ex, ey+1), (ex+1, ey+1) of slab ez; a word is rho
-// rounded to a 22-bit mantissa with the material index in the two freed bits
-// (n_mat > 1).  Slabs linear; inside a slab 4 (x) x 2 (y) tiles of 8 elements.
+// voxels (ex, ey), (ex+1, ey), (ex, ey+1), (ex+1, ey+1) of slab ez.  With more than
+// one material a word is rho rounded to a 21-bit mantissa with tags in the three
+// freed bits: bits 0-1 the material index; bit 2, in the first word of an element
+// only, "the 8 corners of cell (ex, ey, ez) (this quad and the one above it in slab
+// ez + 1) all have this material".  Element order: packed_lay 0 = slabs linear, 4 (x)
+// x 2 (y) tiles of 8 elements inside a slab; 1 = linear with strides sy, sz.
+// One thread per element slot; slots that are stride padding are zeroed.
 __global__ void __launch_bounds__(256)
 gdrr_ingest_packed_kernel(const IngestParams P) {
-    const size_t total = (size_t)P.px * P.py * P.pz;
+    const size_t total = (size_t)P.sz * P.pz;
     const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= total) return;
-    const int e = (int)(o & 7);
-    size_t t = o >> 3;
-    const int ntx = P.px >> 2, nty = P.py >> 1;
-    const int tx = (int)(t % ntx);
-    t /= ntx;
-    const int ty = (int)(t % nty);
-    const int ez = (int)(t / nty);
-    const int ex = 4 * tx + (e & 3), ey = 2 * ty + (e >> 2);
-    const int iz = min(max(ez - 1, 0), P.nz - 1);
-    unsigned w[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const int ix = min(max(ex + (k & 1) - 1, 0), P.nx - 1);
-        const int iy = min(max(ey + (k >> 1) - 1, 0), P.ny - 1);
-        const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
-        unsigned bits = __float_as_uint(P.rho[src]);
-        const unsigned m = P.mat[src];
-        if ((int)m >= P.n_mat) *P.bad_flag = 1;
-        if (P.n_mat > 1) bits = ((bits + 2u) & ~3u) | (m & 3u);
-        w[k] = bits;
+    const int ez = (int)(o / (size_t)P.sz);
+    const int rs = (int)(o - (size_t)ez * P.sz);
+    int ex, ey;
+    if (P.packed_lay == 0) {
+        const int e = rs & 7, t = rs >> 3, ntx = P.sy >> 3;
+        ex = 4 * (t % ntx) + (e & 3);
+        ey = 2 * (t / ntx) + (e >> 2);
+    } else {
+        ey = rs / P.sy;
+        ex = rs - ey * P.sy;
     }
-    reinterpret_cast<uint4*>(P.vox)[o] = make_uint4(w[0], w[1], w[2], w[3]);
+    uint4 out = make_uint4(0u, 0u, 0u, 0u);
+    if (ex < P.px && ey < P.py) {
+        unsigned w[4];
+        unsigned mixed = 0u, m0 = 0u;
+#pragma unroll
+        for (int dz = 0; dz < 2; ++dz) {
+            const int iz = min(max(ez + dz - 1, 0), P.nz - 1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int ix = min(max(ex + (k & 1) - 1, 0), P.nx - 1);
+                const int iy = min(max(ey + (k >> 1) - 1, 0), P.ny - 1);
+                const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
+                const unsigned m = P.mat[src];
+                if (dz == 0 && k == 0) m0 = m;
+                mixed |= m ^ m0;
+                if (dz == 0) {
+                    unsigned bits = __float_as_uint(P.rho[src]);
+                    if ((int)m >= P.n_mat) *P.bad_flag = 1;
+                    if (P.n_mat > 1) bits = ((bits + 4u) & ~7u) | (m & 3u);
+                    w[k] = bits;
+                }
+            }
+        }
+        if (P.n_mat > 1 && mixed == 0u) w[0] |= 4u;
+        out = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+    reinterpret_cast<uint4*>(P.vox)[o] = out;
 }
 
 template <int VW, int LAYOUT>
@@ -105,7 +125,7 @@ static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
 
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s) {
     if (layout == 2) {
-        const size_t total = (size_t)p.px * p.py * p.pz;
+        const size_t total = (size_t)p.sz * p.pz;
         gdrr_ingest_packed_kernel<<<(unsigned int)((total + 255) / 256), 256, 0, s>>>(p);
         return cudaGetLastError();
     }
