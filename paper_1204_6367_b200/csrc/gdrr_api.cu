@@ -214,6 +214,7 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
         P.v.stride_z = vol->px * vol->py;
     }
     P.v.packed_lay = vol->packed_lay;
+    P.v.vox1 = (const char*)vol->vox + 16 * (size_t)vol->sz;
     P.mu_tab = ctx->mu_dev;
     P.src_tab = ctx->src_dev;
     P.bt_thick = ctx->bt_dev;

@@ -32,6 +32,7 @@ struct GeomParams {
 
 struct VolumeParams {
     const void* vox;                // device, layout below
+    const void* vox1;               // PACKED_QUAD: vox + one slab (its own parameter: one IMAD.WIDE per load)
     int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: 8 * tiles per tile-row
     int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab
     int packed_lay;                 // PACKED_QUAD element order: 0 = 4 x 2 tiles in a slab, 1 = linear with skewed strides

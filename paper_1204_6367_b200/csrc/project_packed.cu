@@ -112,9 +112,75 @@ __device__ __forceinline__ int sample_index(const ChunkBase& b, int idx0, int qx
     return idx0 + (qz >> kFracBits) * sz + (qy >> kFracBits) * sy + (qx >> kFracBits);
 }
 
+
+// State of one ray while it is sampled.
+template <int VW>
+struct RayAcc {
+    float part[VW];     // per-material partial sums of the current chunk
+    float cur;          // running sum of pure cells of material curm4 & 3
+    unsigned curm4;     // 4 | material
+};
+
+struct Sampler {
+    const uint4* __restrict__ vol0;     // slab iz
+    const uint4* __restrict__ vol1;     // slab iz + 1
+    int sy, sz;
+    int dqx, dqy, dqz;
+    unsigned fmask, fone;
+};
+
+// `cnt` consecutive samples of a chunk.  PRED = false: every lane of the warp owns all of
+// them and cnt is even (the common case); PRED = true: sample s is this ray's iff
+// rel + s < un (first and last chunk of the warp).  Two register buffers: the loads of
+// sample s + 1 are in flight while sample s is blended.
+template <int VW, int LAY, bool PRED>
+__device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, int cnt, unsigned rel, unsigned un,
+                                          RayAcc<VW>& A) {
+    int qx = b.qx, qy = b.qy, qz = b.qz;
+    const int idx0 = (LAY == 0) ? 0 : elem_index<1>(b.cx, b.cy, b.cz, S.sy, S.sz);
+    uint4 a0 = make_uint4(0, 0, 0, 0), c0 = a0, a1 = a0, c1 = a0;
+    bool act0 = !PRED || rel < un;
+    if (act0) {
+        const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
+        a0 = __ldg(S.vol0 + idx);
+        c0 = __ldg(S.vol1 + idx);
+    }
+    for (int s = 0; s < cnt; s += 2) {
+        float fx = frac_float(qx, S.fmask, S.fone);
+        float fy = frac_float(qy, S.fmask, S.fone);
+        float fz = frac_float(qz, S.fmask, S.fone);
+        qx += S.dqx; qy += S.dqy; qz += S.dqz;
+        const bool more = !PRED || s + 1 < cnt;                  // warp-uniform
+        const bool act1 = more && (!PRED || rel + 1u < un);
+        if (act1) {
+            const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
+            a1 = __ldg(S.vol0 + idx);
+            c1 = __ldg(S.vol1 + idx);
+        }
+        if (act0) blend_sample<VW>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
+        if (more) {
+            fx = frac_float(qx, S.fmask, S.fone);
+            fy = frac_float(qy, S.fmask, S.fone);
+            fz = frac_float(qz, S.fmask, S.fone);
+            qx += S.dqx; qy += S.dqy; qz += S.dqz;
+            rel += 2u;
+            act0 = (s + 2 < cnt) && (!PRED || rel < un);
+            if (act0) {
+                const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
+                a0 = __ldg(S.vol0 + idx);
+                c0 = __ldg(S.vol1 + idx);
+            }
+            if (act1) blend_sample<VW>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
+        }
+    }
+}
+
 template <int VW, int LAY, int LMAP, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB)
 gdrr_project_packed_kernel(const ProjectParams P) {
+    // the ray's line in index space (6 doubles) is needed once per chunk only: keep it in
+    // shared memory, not in 12 registers of the sampling loop
+    __shared__ double s_line[6][kThreads];
     float4* s_mu;
     float2* s_src;
     load_tables(P, s_mu, s_src);
@@ -126,90 +192,75 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     const bool valid = i < P.g.nu && j < P.g.nv;
 
     // ---- a1: ray setup (fp64) ------------------------------------------------
-    Ray r;
-    ray_setup(P.g, P.g.proj_begin + pl, min(i, P.g.nu - 1), min(j, P.g.nv - 1), r);
-    if (!valid) r.n = 0;
-    if (valid && P.ray_table) {
-        const size_t pix = ((size_t)pl * P.g.nv + j) * P.g.nu + i;
-        reinterpret_cast<int2*>(P.ray_table)[pix] = make_int2(r.j0, r.n);
+    int j0, n;
+    Sampler S;
+    {
+        Ray r;
+        ray_setup(P.g, P.g.proj_begin + pl, min(i, P.g.nu - 1), min(j, P.g.nv - 1), r);
+        if (!valid) r.n = 0;
+        if (valid && P.ray_table) {
+            const size_t pix = ((size_t)pl * P.g.nv + j) * P.g.nu + i;
+            reinterpret_cast<int2*>(P.ray_table)[pix] = make_int2(r.j0, r.n);
+        }
+        double gs[3], dg[3];
+        index_line(P.g, r, gs, dg);
+        S.dqx = __double2int_rn(dg[0] * 8388608.0);
+        S.dqy = __double2int_rn(dg[1] * 8388608.0);
+        S.dqz = __double2int_rn(dg[2] * 8388608.0);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            s_line[a][threadIdx.x] = gs[a];
+            s_line[3 + a][threadIdx.x] = dg[a];
+        }
+        j0 = r.j0;
+        n = r.n;
     }
-    double gs[3], dg[3];
-    index_line(P.g, r, gs, dg);
-    const int dqx = __double2int_rn(dg[0] * 8388608.0);
-    const int dqy = __double2int_rn(dg[1] * 8388608.0);
-    const int dqz = __double2int_rn(dg[2] * 8388608.0);
-
-    const int sy = P.v.stride_y, sz = P.v.stride_z;
-    const uint4* __restrict__ vol0 = reinterpret_cast<const uint4*>(P.v.vox);   // slab iz
-    const uint4* __restrict__ vol1 = vol0 + sz;                                  // slab iz + 1
-    const unsigned fmask = P.frac_mask, fone = P.one_bits;
+    S.sy = P.v.stride_y;
+    S.sz = P.v.stride_z;
+    S.vol0 = reinterpret_cast<const uint4*>(P.v.vox);
+    S.vol1 = reinterpret_cast<const uint4*>(P.v.vox1);
+    S.fmask = P.frac_mask;
+    S.fone = P.one_bits;
 
     // Interval indices k are counted from the source (reading Q9), so all lanes of the
     // warp walk the same k: the warp's samples lie on a sphere around the source.
-    const int kmin = __reduce_min_sync(0xffffffffu, r.n > 0 ? r.j0 : 0x7fffffff);
-    const int kmax = __reduce_max_sync(0xffffffffu, r.n > 0 ? r.j0 + r.n : (int)0x80000000);
-    const unsigned un = (unsigned)r.n;
+    const int kmin = __reduce_min_sync(0xffffffffu, n > 0 ? j0 : 0x7fffffff);
+    const int kmax = __reduce_max_sync(0xffffffffu, n > 0 ? j0 + n : (int)0x80000000);
+    const unsigned un = (unsigned)n;
     const int CH = P.chunk;
 
     // ---- a2-a4: sampling -------------------------------------------------------
     float acc[VW];
 #pragma unroll
     for (int m = 0; m < VW; ++m) acc[m] = 0.f;
-    unsigned curm4 = 4u;       // 4 | material of the running sum of pure cells
-    float cur = 0.f;
+    RayAcc<VW> A;
+    A.cur = 0.f;
+    A.curm4 = 4u;
 
     for (int kc = (kmin / CH) * CH; kc < kmax; kc += CH) {
         const int s0 = max(kmin - kc, 0);
         const int cnt = min(kmax - kc, CH) - s0;
+        double gs[3], dg[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            gs[a] = s_line[a][threadIdx.x];
+            dg[a] = s_line[3 + a][threadIdx.x];
+        }
         const ChunkBase b = chunk_base(gs, dg, kc + s0);
-        int qx = b.qx, qy = b.qy, qz = b.qz;
-        const int idx0 = (LAY == 0) ? 0 : elem_index<1>(b.cx, b.cy, b.cz, sy, sz);
-        unsigned rel = (unsigned)(kc + s0 - r.j0);      // sample s of the chunk is this ray's iff rel + s < n
-
-        float part[VW];
+        const unsigned rel = (unsigned)(kc + s0 - j0);
 #pragma unroll
-        for (int m = 0; m < VW; ++m) part[m] = 0.f;
+        for (int m = 0; m < VW; ++m) A.part[m] = 0.f;
 
-        // two register buffers: the loads of sample s + 1 are in flight while sample s is blended
-        uint4 a0 = make_uint4(0, 0, 0, 0), c0 = a0, a1 = a0, c1 = a0;
-        bool act0 = rel < un;
-        if (act0) {
-            const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, sy, sz);
-            a0 = __ldg(vol0 + idx);
-            c0 = __ldg(vol1 + idx);
-        }
-        for (int s = 0; s < cnt; s += 2) {
-            float fx = frac_float(qx, fmask, fone);
-            float fy = frac_float(qy, fmask, fone);
-            float fz = frac_float(qz, fmask, fone);
-            qx += dqx; qy += dqy; qz += dqz;
-            const bool more = s + 1 < cnt;                       // warp-uniform
-            const bool act1 = more && (rel + 1u < un);
-            if (act1) {
-                const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, sy, sz);
-                a1 = __ldg(vol0 + idx);
-                c1 = __ldg(vol1 + idx);
-            }
-            if (act0) blend_sample<VW>(a0, c0, fx, fy, fz, cur, curm4, part);
-            if (more) {
-                fx = frac_float(qx, fmask, fone);
-                fy = frac_float(qy, fmask, fone);
-                fz = frac_float(qz, fmask, fone);
-                qx += dqx; qy += dqy; qz += dqz;
-                rel += 2u;
-                act0 = (s + 2 < cnt) && (rel < un);
-                if (act0) {
-                    const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, sy, sz);
-                    a0 = __ldg(vol0 + idx);
-                    c0 = __ldg(vol1 + idx);
-                }
-                if (act1) blend_sample<VW>(a1, c1, fx, fy, fz, cur, curm4, part);
-            }
-        }
-        add_routed<VW>(part, (int)(curm4 & 3u), cur);
-        cur = 0.f;
+        const bool mine = rel < un && rel + (unsigned)cnt <= un;         // this lane owns the whole chunk
+        if (__all_sync(0xffffffffu, mine) && !(cnt & 1))
+            run_chunk<VW, LAY, false>(S, b, cnt, rel, un, A);
+        else
+            run_chunk<VW, LAY, true>(S, b, cnt, rel, un, A);
+
+        add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur);
+        A.cur = 0.f;
 #pragma unroll
-        for (int m = 0; m < VW; ++m) acc[m] += part[m];
+        for (int m = 0; m < VW; ++m) acc[m] += A.part[m];
     }
 
     if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
@@ -225,7 +276,7 @@ static cudaError_t launch_packed_t(const ProjectParams& p, cudaStream_t s) {
 
 template <int VW, int LAY>
 static cudaError_t launch_packed_l(const ProjectParams& p, int variant, cudaStream_t s) {
-    const int lmap = (variant >> 1) & 1, occ = (variant >> 2) & 3;
+    const int lmap = ((variant >> 1) & 1) ^ 1, occ = (variant >> 2) & 3;
     if (lmap == 0) {
         if (occ == 1) return launch_packed_t<VW, LAY, 0, 3>(p, s);
         if (occ == 2) return launch_packed_t<VW, LAY, 0, 5>(p, s);
