@@ -4,7 +4,7 @@
 // bits carry tags (n_materials > 1): bits 0-1 the material index, bit 2 (first
 // word of an element only) "all 8 corners of this cell have this material".
 // Element (ix, iy, iz) of the device volume is the 2x2 quad of words
-// {(ix,iy), (ix+1,iy), (ix,iy+1), (ix+1,iy+1)} of slab iz, stored for EVERY
+// {(ix,iy), (ix,iy+1), (ix+1,iy), (ix+1,iy+1)} of slab iz, stored for EVERY
 // (ix, iy) (quads overlap, 16 B per voxel).  A sample needs two 16-byte loads
 // (slabs iz and iz+1).
 //
@@ -30,6 +30,10 @@
 // material (a denormal bit pattern) contributes exactly 0.
 #include "project_common.cuh"
 
+#ifndef GDRR_L2_PREFETCH
+#define GDRR_L2_PREFETCH 0
+#endif
+
 namespace gdrr {
 
 template <int VW>
@@ -39,6 +43,37 @@ __device__ __forceinline__ void add_routed(float (&part)[VW], int m, float v) {
 }
 
 __device__ __forceinline__ float lerp(float a, float b, float t) { return fmaf(t, b - a, a); }
+
+// Packed fp32 pairs (sm_100 FADD2 / FFMA2: two fp32 lanes per instruction, same rounding as the
+// scalar forms; .ftz as the rest of the library).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(unsigned lo, unsigned hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+__device__ __forceinline__ f32x2 bcast2(float v) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(r) : "f"(v));
+    return r;
+}
+__device__ __forceinline__ f32x2 lerp2(f32x2 a, f32x2 b, f32x2 t) {       // a + t (b - a), per lane
+    f32x2 d, r;
+    asm("sub.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(b), "l"(a));
+    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(t), "l"(d), "l"(a));
+    return r;
+}
+// Tri-linear blend of one cell.  Words of a quad: (x0y0, x0y1, x1y0, x1y1), so that the two
+// x-lerps of a slab are one packed lerp between its register pairs, the two z-lerps another.
+__device__ __forceinline__ float blend_cell(const uint4& a, const uint4& c, float fx, float fy, float fz) {
+    const f32x2 tx = bcast2(fx), tz = bcast2(fz);
+    const f32x2 va = lerp2(pack2(a.x, a.y), pack2(a.z, a.w), tx);       // slab iz:     (y0, y1) at x
+    const f32x2 vc = lerp2(pack2(c.x, c.y), pack2(c.z, c.w), tx);       // slab iz + 1
+    const f32x2 v = lerp2(va, vc, tz);                                  // (y0, y1) at (x, z)
+    float y0, y1;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(y0), "=f"(y1) : "l"(v));
+    return lerp(y0, y1, fy);
+}
 
 // (q & mask) | one in a single LOP3; mask and one arrive as kernel parameters so
 // that they live in registers instead of being split into two immediate ops.
@@ -72,28 +107,33 @@ __device__ __forceinline__ int elem_index(int cx, int cy, int cz, int sy, int sz
 
 // One sample: blend the 8 corners (a = slab iz, c = slab iz + 1) with the
 // fractions (fx, fy, fz) and add to the running sums.
-template <int VW>
+// UNI: every lane of the warp is here (unpredicated chunk): vote, so that the common case "all lanes
+// in a pure cell of their running material" is a warp-uniform branch without reconvergence overhead.
+template <int VW, bool UNI>
 __device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, float fx, float fy, float fz,
                                              float& cur, unsigned& curm4, float (&part)[VW]) {
     bool fast = true;
     if (VW > 1) fast = (a.x & 7u) == curm4;        // pure cell of the running material
+    if (VW > 1 && UNI) {
+        if (__all_sync(0xffffffffu, fast)) {
+            cur += blend_cell(a, c, fx, fy, fz);
+            return;
+        }
+    }
     if (fast) {
-        const float v0 = lerp(lerp(__uint_as_float(a.x), __uint_as_float(a.y), fx),
-                              lerp(__uint_as_float(a.z), __uint_as_float(a.w), fx), fy);
-        const float v1 = lerp(lerp(__uint_as_float(c.x), __uint_as_float(c.y), fx),
-                              lerp(__uint_as_float(c.z), __uint_as_float(c.w), fx), fy);
-        cur += lerp(v0, v1, fz);
+        cur += blend_cell(a, c, fx, fy, fz);
     } else {
         // mixed cell, or a pure cell of another material: route every weighted corner
         const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
         const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
+        // w<y><z>; words (x0y0, x0y1, x1y0, x1y1)
         add_routed<VW>(part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
-        add_routed<VW>(part, (int)(a.y & 3u), fx * w00 * __uint_as_float(a.y));
-        add_routed<VW>(part, (int)(a.z & 3u), gx * w10 * __uint_as_float(a.z));
+        add_routed<VW>(part, (int)(a.y & 3u), gx * w10 * __uint_as_float(a.y));
+        add_routed<VW>(part, (int)(a.z & 3u), fx * w00 * __uint_as_float(a.z));
         add_routed<VW>(part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
         add_routed<VW>(part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
-        add_routed<VW>(part, (int)(c.y & 3u), fx * w01 * __uint_as_float(c.y));
-        add_routed<VW>(part, (int)(c.z & 3u), gx * w11 * __uint_as_float(c.z));
+        add_routed<VW>(part, (int)(c.y & 3u), gx * w11 * __uint_as_float(c.y));
+        add_routed<VW>(part, (int)(c.z & 3u), fx * w01 * __uint_as_float(c.z));
         add_routed<VW>(part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
         // the running sum follows the material the ray is now in
         const unsigned m4 = (c.w & 3u) | 4u;
@@ -103,6 +143,20 @@ __device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, flo
             curm4 = m4;
         }
     }
+}
+
+// 16-byte read-only load; the L2 is asked to fetch the whole 256-byte neighbourhood on a miss
+// (the x-run of 16 elements the neighbouring lanes and the next steps are about to need).
+__device__ __forceinline__ uint4 ld_quad(const uint4* p) {
+    uint4 v;
+#if GDRR_L2_PREFETCH == 256
+    asm("ld.global.nc.L2::256B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+#elif GDRR_L2_PREFETCH == 128
+    asm("ld.global.nc.L2::128B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+#else
+    v = __ldg(p);
+#endif
+    return v;
 }
 
 template <int LAY>
@@ -142,8 +196,8 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
     bool act0 = !PRED || rel < un;
     if (act0) {
         const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
-        a0 = __ldg(S.vol0 + idx);
-        c0 = __ldg(S.vol1 + idx);
+        a0 = ld_quad(S.vol0 + idx);
+        c0 = ld_quad(S.vol1 + idx);
     }
     for (int s = 0; s < cnt; s += 2) {
         float fx = frac_float(qx, S.fmask, S.fone);
@@ -154,10 +208,10 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
         const bool act1 = more && (!PRED || rel + 1u < un);
         if (act1) {
             const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
-            a1 = __ldg(S.vol0 + idx);
-            c1 = __ldg(S.vol1 + idx);
+            a1 = ld_quad(S.vol0 + idx);
+            c1 = ld_quad(S.vol1 + idx);
         }
-        if (act0) blend_sample<VW>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
+        if (act0) blend_sample<VW, !PRED>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
         if (more) {
             fx = frac_float(qx, S.fmask, S.fone);
             fy = frac_float(qy, S.fmask, S.fone);
@@ -167,10 +221,10 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
             act0 = (s + 2 < cnt) && (!PRED || rel < un);
             if (act0) {
                 const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
-                a0 = __ldg(S.vol0 + idx);
-                c0 = __ldg(S.vol1 + idx);
+                a0 = ld_quad(S.vol0 + idx);
+                c0 = ld_quad(S.vol1 + idx);
             }
-            if (act1) blend_sample<VW>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
+            if (act1) blend_sample<VW, !PRED>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
         }
     }
 }

@@ -63,7 +63,7 @@ gdrr_ingest_kernel(const IngestParams P) {
 }
 
 // PACKED_QUAD (project_packed.cu): element (ex, ey, ez) = the four words of stored
-// voxels (ex, ey), (ex+1, ey), (ex, ey+1), (ex+1, ey+1) of slab ez.  With more than
+// voxels (ex, ey), (ex, ey+1), (ex+1, ey), (ex+1, ey+1) of slab ez.  With more than
 // one material a word is rho rounded to a 21-bit mantissa with tags in the three
 // freed bits: bits 0-1 the material index; bit 2, in the first word of an element
 // only, "the 8 corners of cell (ex, ey, ez) (this quad and the one above it in slab
@@ -95,8 +95,8 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
             const int iz = min(max(ez + dz - 1, 0), P.nz - 1);
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const int ix = min(max(ex + (k & 1) - 1, 0), P.nx - 1);
-                const int iy = min(max(ey + (k >> 1) - 1, 0), P.ny - 1);
+                const int ix = min(max(ex + (k >> 1) - 1, 0), P.nx - 1);
+                const int iy = min(max(ey + (k & 1) - 1, 0), P.ny - 1);
                 const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
                 const unsigned m = P.mat[src];
                 if (dz == 0 && k == 0) m0 = m;
