@@ -39,7 +39,6 @@ struct gdrr_context {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
-    int variant = 0;            // kernel variant under exploration (GDRR_VARIANT), 0 = default
 };
 
 struct gdrr_volume {
@@ -48,7 +47,7 @@ struct gdrr_volume {
     int nx, ny, nz, px, py, pz;
     double d[3], c[3];
     int n_mat, vw, layout;
-    int sy, sz, packed_lay;     // PACKED_QUAD: element strides and order
+    int sy, sz;                 // PACKED_QUAD: element strides
 };
 
 static thread_local std::string g_create_err;
@@ -87,11 +86,11 @@ struct DeviceGuard {
 int vector_width(int n_mat) { return n_mat <= 1 ? 1 : (n_mat == 2 ? 2 : 4); }
 
 // Stored dims of the device volume: voxels N + 2 rounded up to even (BRICK, LINEAR);
-// quads (N + 1 rounded up to the 4 x 2 tile) x (N + 2 slabs) for PACKED_QUAD.
+// quads (N + 1) x (N + 1) x (N + 2 slabs) for PACKED_QUAD.
 void stored_dims(int nx, int ny, int nz, int layout, int& px, int& py, int& pz) {
     if (layout == GDRR_LAYOUT_PACKED_QUAD) {
-        px = (nx + 1 + 3) & ~3;
-        py = (ny + 1 + 1) & ~1;
+        px = nx + 1;
+        py = ny + 1;
         pz = nz + 2;
     } else {
         px = (nx + 3) & ~1;
@@ -100,25 +99,19 @@ void stored_dims(int nx, int ny, int nz, int layout, int& px, int& py, int& pz) 
     }
 }
 
-// PACKED_QUAD element strides.  Order 0: slabs linear, 4 x 2 tiles of 8 elements in a slab
-// (px, py already rounded to the tile).  Order 1: linear with row stride = 3 and slab stride
-// = 4 (mod 8), so that neighbouring elements fall in different 16-byte bank groups of the L1
-// data RAM in every direction (project_packed.cu).
-void packed_strides(int px, int py, int lay, int& sy, int& sz) {
-    if (lay == 0) {
-        sy = 8 * (px / 4);
-        sz = px * py;
-    } else {
-        sy = px + ((3 - px % 8) + 8) % 8;
-        const long long s0 = (long long)sy * py;
-        sz = (int)(s0 + ((4 - s0 % 8) + 8) % 8);
-    }
+// PACKED_QUAD element strides: linear, with the row stride = 3 and the slab stride = 4 (mod 8),
+// so that neighbouring elements fall in different 16-byte bank groups of the L1 data RAM in
+// every direction (project_packed.cu).
+void packed_strides(int px, int py, int& sy, int& sz) {
+    sy = px + ((3 - px % 8) + 8) % 8;
+    const long long s0 = (long long)sy * py;
+    sz = (int)(s0 + ((4 - s0 % 8) + 8) % 8);
 }
 
-size_t packed_elements(int nx, int ny, int nz, int lay) {
+size_t packed_elements(int nx, int ny, int nz) {
     int px, py, pz, sy, sz;
     stored_dims(nx, ny, nz, GDRR_LAYOUT_PACKED_QUAD, px, py, pz);
-    packed_strides(px, py, lay, sy, sz);
+    packed_strides(px, py, sy, sz);
     return (size_t)sz * pz;
 }
 
@@ -147,7 +140,7 @@ int check_dims(gdrr_context* ctx, int nx, int ny, int nz, int n_materials, int l
     stored_dims(nx, ny, nz, layout, px, py, pz);
     double total = (double)px * py * pz;
     if (layout == GDRR_LAYOUT_PACKED_QUAD)
-        total = (double)std::max(packed_elements(nx, ny, nz, 0), packed_elements(nx, ny, nz, 1)) + px * (double)py;
+        total = (double)packed_elements(nx, ny, nz) + px * (double)py;
     if (total >= 2147483648.0)
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "padded volume has %.0f voxels; the sampler indexes with int32", total);
     return GDRR_OK;
@@ -213,7 +206,6 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
         P.v.stride_y = vol->px;
         P.v.stride_z = vol->px * vol->py;
     }
-    P.v.packed_lay = vol->packed_lay;
     P.v.vox1 = (const char*)vol->vox + 16 * (size_t)vol->sz;
     P.mu_tab = ctx->mu_dev;
     P.src_tab = ctx->src_dev;
@@ -235,7 +227,7 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
 }
 
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
-    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, vol->ctx->variant, s);
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);
 }
 
@@ -256,7 +248,6 @@ int gdrr_create_context(int cuda_device, gdrr_context** out) {
     gdrr_context* ctx = new (std::nothrow) gdrr_context;
     if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "out of host memory");
     ctx->device = cuda_device;
-    if (const char* v = std::getenv("GDRR_VARIANT")) ctx->variant = std::atoi(v);
     DeviceGuard guard(cuda_device);
     if (guard.status != cudaSuccess) { delete ctx; return cuda_fail(nullptr, guard.status, "cudaSetDevice"); }
     e = cudaMalloc(&ctx->flag_dev, sizeof(int));
@@ -292,8 +283,7 @@ int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int lay
     int px, py, pz;
     stored_dims(nx, ny, nz, layout, px, py, pz);
     *bytes = (size_t)px * py * pz * element_bytes(n_materials, layout);
-    if (layout == GDRR_LAYOUT_PACKED_QUAD)      // either element order fits
-        *bytes = 16 * std::max(packed_elements(nx, ny, nz, 0), packed_elements(nx, ny, nz, 1));
+    if (layout == GDRR_LAYOUT_PACKED_QUAD) *bytes = 16 * packed_elements(nx, ny, nz);
     return GDRR_OK;
 }
 
@@ -330,8 +320,7 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     stored_dims(nx, ny, nz, layout, ip.px, ip.py, ip.pz);
     ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev;
     ip.sy = ip.sz = 0;
-    ip.packed_lay = (ctx->variant & 1) ? 0 : 1;
-    if (layout == GDRR_LAYOUT_PACKED_QUAD) packed_strides(ip.px, ip.py, ip.packed_lay, ip.sy, ip.sz);
+    if (layout == GDRR_LAYOUT_PACKED_QUAD) packed_strides(ip.px, ip.py, ip.sy, ip.sz);
     const int vw = vector_width(n_materials);
     e = launch_ingest(ip, vw, layout, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel launch");
@@ -349,7 +338,7 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     v->d[0] = dx_mm; v->d[1] = dy_mm; v->d[2] = dz_mm;
     for (int a = 0; a < 3; ++a) v->c[a] = centre_mm ? centre_mm[a] : 0.0;
     v->n_mat = n_materials; v->vw = vw; v->layout = layout;
-    v->sy = ip.sy; v->sz = ip.sz; v->packed_lay = ip.packed_lay;
+    v->sy = ip.sy; v->sz = ip.sz;
     *out = v;
     return GDRR_OK;
 }

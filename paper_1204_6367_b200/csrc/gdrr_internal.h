@@ -6,9 +6,8 @@
 
 namespace gdrr {
 
-// Tile of detector pixels one CTA owns: 16 x 16, eight warps of 8 (u) x 4 (v)
-// pixels each.  A warp's rays then cross the volume as a beam about 4 x 1.6
-// voxels wide at C3.
+// Tile of detector pixels one CTA owns: 16 x 16, eight warps (8 (u) x 4 (v) pixels
+// each in the exact-layout kernels, 4 x 8 in the packed sampler).
 constexpr int kTileU = 16;
 constexpr int kTileV = 16;
 constexpr int kThreads = kTileU * kTileV;
@@ -33,9 +32,8 @@ struct GeomParams {
 struct VolumeParams {
     const void* vox;                // device, layout below
     const void* vox1;               // PACKED_QUAD: vox + one slab (its own parameter: one IMAD.WIDE per load)
-    int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: 8 * tiles per tile-row
-    int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab
-    int packed_lay;                 // PACKED_QUAD element order: 0 = 4 x 2 tiles in a slab, 1 = linear with skewed strides
+    int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: elements per row (= 3 mod 8)
+    int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab (= 4 mod 8)
 };
 
 struct ProjectParams {
@@ -59,7 +57,7 @@ struct IngestParams {
     void* vox;
     int nx, ny, nz;
     int px, py, pz;                 // stored dims (voxels for BRICK / LINEAR, quads for PACKED_QUAD)
-    int sy, sz, packed_lay;         // PACKED_QUAD: element strides and order (VolumeParams)
+    int sy, sz;                     // PACKED_QUAD: element strides (VolumeParams)
     int n_mat;
     int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
 };
@@ -67,7 +65,7 @@ struct IngestParams {
 // Host-callable launchers (each returns the cudaGetLastError() of its launch).
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
-cudaError_t launch_project_packed(const ProjectParams& p, int vw, int variant, cudaStream_t s);
+cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 

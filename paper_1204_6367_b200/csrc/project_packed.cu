@@ -30,10 +30,6 @@
 // material (a denormal bit pattern) contributes exactly 0.
 #include "project_common.cuh"
 
-#ifndef GDRR_L2_PREFETCH
-#define GDRR_L2_PREFETCH 0
-#endif
-
 namespace gdrr {
 
 template <int VW>
@@ -83,30 +79,19 @@ __device__ __forceinline__ float frac_float(int q, unsigned mask, unsigned one) 
     return __uint_as_float(o) - 1.f;
 }
 
-// thread -> pixel.  LMAP 0: a warp is 8 (u) x 4 (v) pixels, a load phase (8 lanes)
-// one row of 8; LMAP 1: a warp is 4 (u) x 8 (v), a phase 4 x 2 pixels.
-template <int LMAP>
+// thread -> pixel: a warp is 4 (u) x 8 (v) pixels, so that a load phase (8 consecutive lanes) is a
+// compact 4 x 2 patch of rays; the CTA's 16 x 16 tile is 4 x 2 warps.
 __device__ __forceinline__ void thread_pixel_map(int& i, int& j) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (LMAP == 0) {
-        i = blockIdx.x * kTileU + (warp & 1) * 8 + (lane & 7);
-        j = blockIdx.y * kTileV + (warp >> 1) * 4 + (lane >> 3);
-    } else {
-        i = blockIdx.x * kTileU + (warp & 3) * 4 + (lane & 3);
-        j = blockIdx.y * kTileV + (warp >> 2) * 8 + (lane >> 2);
-    }
+    i = blockIdx.x * kTileU + (warp & 3) * 4 + (lane & 3);
+    j = blockIdx.y * kTileV + (warp >> 2) * 8 + (lane >> 2);
 }
 
-// Element index of cell (cx, cy, cz).  LAY 0: 4 (x) x 2 (y) tiles of 8 elements
-// inside a slab; LAY 1: linear, skewed strides.
-template <int LAY>
+// Element index of cell (cx, cy, cz): linear, strides sy = 3 and sz = 4 (mod 8).
 __device__ __forceinline__ int elem_index(int cx, int cy, int cz, int sy, int sz) {
-    if (LAY == 0) return cz * sz + (cy >> 1) * sy + ((cy & 1) << 2) + cx + (cx & ~3);
     return cz * sz + cy * sy + cx;
 }
 
-// One sample: blend the 8 corners (a = slab iz, c = slab iz + 1) with the
-// fractions (fx, fy, fz) and add to the running sums.
 // UNI: every lane of the warp is here (unpredicated chunk): vote, so that the common case "all lanes
 // in a pure cell of their running material" is a warp-uniform branch without reconvergence overhead.
 template <int VW, bool UNI>
@@ -145,27 +130,10 @@ __device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, flo
     }
 }
 
-// 16-byte read-only load; the L2 is asked to fetch the whole 256-byte neighbourhood on a miss
-// (the x-run of 16 elements the neighbouring lanes and the next steps are about to need).
-__device__ __forceinline__ uint4 ld_quad(const uint4* p) {
-    uint4 v;
-#if GDRR_L2_PREFETCH == 256
-    asm("ld.global.nc.L2::256B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-#elif GDRR_L2_PREFETCH == 128
-    asm("ld.global.nc.L2::128B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-#else
-    v = __ldg(p);
-#endif
-    return v;
-}
-
-template <int LAY>
-__device__ __forceinline__ int sample_index(const ChunkBase& b, int idx0, int qx, int qy, int qz, int sy, int sz) {
-    if (LAY == 0)
-        return elem_index<0>(b.cx + (qx >> kFracBits), b.cy + (qy >> kFracBits), b.cz + (qz >> kFracBits), sy, sz);
+// element of the sample at in-chunk fixed-point position q (idx0 = element of the chunk's base cell)
+__device__ __forceinline__ int sample_index(int idx0, int qx, int qy, int qz, int sy, int sz) {
     return idx0 + (qz >> kFracBits) * sz + (qy >> kFracBits) * sy + (qx >> kFracBits);
 }
-
 
 // State of one ray while it is sampled.
 template <int VW>
@@ -187,17 +155,17 @@ struct Sampler {
 // them and cnt is even (the common case); PRED = true: sample s is this ray's iff
 // rel + s < un (first and last chunk of the warp).  Two register buffers: the loads of
 // sample s + 1 are in flight while sample s is blended.
-template <int VW, int LAY, bool PRED>
+template <int VW, bool PRED>
 __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, int cnt, unsigned rel, unsigned un,
                                           RayAcc<VW>& A) {
     int qx = b.qx, qy = b.qy, qz = b.qz;
-    const int idx0 = (LAY == 0) ? 0 : elem_index<1>(b.cx, b.cy, b.cz, S.sy, S.sz);
+    const int idx0 = elem_index(b.cx, b.cy, b.cz, S.sy, S.sz);
     uint4 a0 = make_uint4(0, 0, 0, 0), c0 = a0, a1 = a0, c1 = a0;
     bool act0 = !PRED || rel < un;
     if (act0) {
-        const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
-        a0 = ld_quad(S.vol0 + idx);
-        c0 = ld_quad(S.vol1 + idx);
+        const int idx = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
+        a0 = __ldg(S.vol0 + idx);
+        c0 = __ldg(S.vol1 + idx);
     }
     for (int s = 0; s < cnt; s += 2) {
         float fx = frac_float(qx, S.fmask, S.fone);
@@ -207,9 +175,9 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
         const bool more = !PRED || s + 1 < cnt;                  // warp-uniform
         const bool act1 = more && (!PRED || rel + 1u < un);
         if (act1) {
-            const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
-            a1 = ld_quad(S.vol0 + idx);
-            c1 = ld_quad(S.vol1 + idx);
+            const int idx = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
+            a1 = __ldg(S.vol0 + idx);
+            c1 = __ldg(S.vol1 + idx);
         }
         if (act0) blend_sample<VW, !PRED>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
         if (more) {
@@ -220,17 +188,17 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
             rel += 2u;
             act0 = (s + 2 < cnt) && (!PRED || rel < un);
             if (act0) {
-                const int idx = sample_index<LAY>(b, idx0, qx, qy, qz, S.sy, S.sz);
-                a0 = ld_quad(S.vol0 + idx);
-                c0 = ld_quad(S.vol1 + idx);
+                const int idx = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
+                a0 = __ldg(S.vol0 + idx);
+                c0 = __ldg(S.vol1 + idx);
             }
             if (act1) blend_sample<VW, !PRED>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
         }
     }
 }
 
-template <int VW, int LAY, int LMAP, int MINB>
-__global__ void __launch_bounds__(kThreads, MINB)
+template <int VW>
+__global__ void __launch_bounds__(kThreads, 4)
 gdrr_project_packed_kernel(const ProjectParams P) {
     // the ray's line in index space (6 doubles) is needed once per chunk only: keep it in
     // shared memory, not in 12 registers of the sampling loop
@@ -240,7 +208,7 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     load_tables(P, s_mu, s_src);
 
     int i, j;
-    thread_pixel_map<LMAP>(i, j);
+    thread_pixel_map(i, j);
     const int pl = blockIdx.z;
     // lanes outside the detector stay in the warp (the loop below is warp-synchronous) with n = 0
     const bool valid = i < P.g.nu && j < P.g.nv;
@@ -307,9 +275,9 @@ gdrr_project_packed_kernel(const ProjectParams P) {
 
         const bool mine = rel < un && rel + (unsigned)cnt <= un;         // this lane owns the whole chunk
         if (__all_sync(0xffffffffu, mine) && !(cnt & 1))
-            run_chunk<VW, LAY, false>(S, b, cnt, rel, un, A);
+            run_chunk<VW, false>(S, b, cnt, rel, un, A);
         else
-            run_chunk<VW, LAY, true>(S, b, cnt, rel, un, A);
+            run_chunk<VW, true>(S, b, cnt, rel, un, A);
 
         add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur);
         A.cur = 0.f;
@@ -320,38 +288,18 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
 }
 
-template <int VW, int LAY, int LMAP, int MINB>
+template <int VW>
 static cudaError_t launch_packed_t(const ProjectParams& p, cudaStream_t s) {
     dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
     const size_t smem = (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
-    gdrr_project_packed_kernel<VW, LAY, LMAP, MINB><<<grid, kThreads, smem, s>>>(p);
+    gdrr_project_packed_kernel<VW><<<grid, kThreads, smem, s>>>(p);
     return cudaGetLastError();
 }
 
-template <int VW, int LAY>
-static cudaError_t launch_packed_l(const ProjectParams& p, int variant, cudaStream_t s) {
-    const int lmap = ((variant >> 1) & 1) ^ 1, occ = (variant >> 2) & 3;
-    if (lmap == 0) {
-        if (occ == 1) return launch_packed_t<VW, LAY, 0, 3>(p, s);
-        if (occ == 2) return launch_packed_t<VW, LAY, 0, 5>(p, s);
-        return launch_packed_t<VW, LAY, 0, 4>(p, s);
-    }
-    if (occ == 1) return launch_packed_t<VW, LAY, 1, 3>(p, s);
-    if (occ == 2) return launch_packed_t<VW, LAY, 1, 5>(p, s);
-    return launch_packed_t<VW, LAY, 1, 4>(p, s);
-}
-
-// variant: bit 1 = lane map, bits 2-3 = occupancy target; the element order (p.v.packed_lay)
-// is a property of the ingested volume.
-cudaError_t launch_project_packed(const ProjectParams& p, int vw, int variant, cudaStream_t s) {
-    if (p.v.packed_lay == 0) {
-        if (vw == 1) return launch_packed_l<1, 0>(p, variant, s);
-        if (vw == 2) return launch_packed_l<2, 0>(p, variant, s);
-        return launch_packed_l<4, 0>(p, variant, s);
-    }
-    if (vw == 1) return launch_packed_l<1, 1>(p, variant, s);
-    if (vw == 2) return launch_packed_l<2, 1>(p, variant, s);
-    return launch_packed_l<4, 1>(p, variant, s);
+cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s) {
+    if (vw == 1) return launch_packed_t<1>(p, s);
+    if (vw == 2) return launch_packed_t<2>(p, s);
+    return launch_packed_t<4>(p, s);
 }
 
 }  // namespace gdrr

@@ -67,8 +67,7 @@ gdrr_ingest_kernel(const IngestParams P) {
 // one material a word is rho rounded to a 21-bit mantissa with tags in the three
 // freed bits: bits 0-1 the material index; bit 2, in the first word of an element
 // only, "the 8 corners of cell (ex, ey, ez) (this quad and the one above it in slab
-// ez + 1) all have this material".  Element order: packed_lay 0 = slabs linear, 4 (x)
-// x 2 (y) tiles of 8 elements inside a slab; 1 = linear with strides sy, sz.
+// ez + 1) all have this material".  Elements are stored linearly with strides sy, sz.
 // One thread per element slot; slots that are stride padding are zeroed.
 __global__ void __launch_bounds__(256)
 gdrr_ingest_packed_kernel(const IngestParams P) {
@@ -77,15 +76,8 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
     if (o >= total) return;
     const int ez = (int)(o / (size_t)P.sz);
     const int rs = (int)(o - (size_t)ez * P.sz);
-    int ex, ey;
-    if (P.packed_lay == 0) {
-        const int e = rs & 7, t = rs >> 3, ntx = P.sy >> 3;
-        ex = 4 * (t % ntx) + (e & 3);
-        ey = 2 * (t / ntx) + (e >> 2);
-    } else {
-        ey = rs / P.sy;
-        ex = rs - ey * P.sy;
-    }
+    const int ey = rs / P.sy;
+    const int ex = rs - ey * P.sy;
     uint4 out = make_uint4(0u, 0u, 0u, 0u);
     if (ex < P.px && ey < P.py) {
         unsigned w[4];
