@@ -121,6 +121,7 @@ def time_oracle(w, pix):
     t0 = time.perf_counter()
     out = oracle.project(w, pixels=pix, want_li=False)
     dt = time.perf_counter() - t0
+    time_oracle.last_signal = out["signal"]                 # for the parity figure printed beside the timing
     return int(out["ray_table"][:, 1].sum()), dt, oracle.n_threads_available()
 
 
@@ -196,7 +197,10 @@ def run_b200(args):
     per_gpu = w0.n_proj if args.projections <= 0 else args.projections
     n_total = per_gpu * world
     mine = gd.strided_shard(n_total, world, rank)
-    w = w0.with_phis(gd.scan_angles(n_total)[mine])
+    if args.angle_deg is None:
+        w = w0.with_phis(gd.scan_angles(n_total)[mine])
+    else:                                                   # profiling aid: every projection at one angle
+        w = w0.with_phis(np.full(per_gpu, np.deg2rad(args.angle_deg)))
     launch_proj = per_gpu if args.launch_proj <= 0 else min(args.launch_proj, per_gpu)
 
     pr = g.Projector(w, device=local_rank, layout=args.layout)
@@ -317,8 +321,11 @@ def run_b200(args):
     if not args.no_cpu_baseline:
         pix, sample = sized_oracle_sample(w, args.cpu_seconds)
         n, dt, cores = time_oracle(w, pix)
+        ref = time_oracle.last_signal
+        got = signal.cpu().numpy()[pix[:, 0], pix[:, 2], pix[:, 1]].astype(np.float64)
         cpu = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
-               "sample": f"{sample} ({n} samples)"}
+               "sample": f"{sample} ({n} samples)",
+               "max_rel_err_of_b200_signal_on_sample": float(np.max(np.abs(got - ref) / ref))}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
@@ -342,6 +349,8 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--projections", type=int, default=0, help="projections per GPU (0 = the workload's)")
     ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
+    ap.add_argument("--angle-deg", type=float, default=None,
+                    help="profiling aid: all projections at this one gantry angle instead of an evenly spaced scan")
     ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
