@@ -40,7 +40,7 @@ def _load():
         build()
         _lib = ctypes.CDLL(_LIB)
         for name in ("gdrr_oracle_ray", "gdrr_oracle_trilinear", "gdrr_oracle_ray_samples",
-                     "gdrr_oracle_project", "gdrr_oracle_project_literal"):
+                     "gdrr_oracle_project", "gdrr_oracle_project_siddon", "gdrr_oracle_project_literal"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -132,8 +132,10 @@ def _project_common(w, step):
     return keep, args
 
 
-def project(w, pixels=None, step=None, want_li=True, want_table=True, n_threads=0):
-    """Run the oracle on workload-like ``w``.
+def project(w, pixels=None, step=None, want_li=True, want_table=True, n_threads=0, method="trilinear"):
+    """Run the oracle on workload-like ``w``.  method: "trilinear" (the paper's default
+    midpoint rule) or "siddon" (exact radiological path through homogeneous voxels; the
+    result then also holds ``n_segments``).
 
     pixels: None (every pixel of every projection) or int array [n][3] of
     (projection, column i, row j).  Returns dict(signal, line_integrals,
@@ -154,14 +156,21 @@ def project(w, pixels=None, step=None, want_li=True, want_table=True, n_threads=
         signal = np.zeros(n_pix)
         li = np.zeros((n_pix, M)) if want_li else None
         tab = np.zeros((n_pix, 2), dtype=np.int32) if want_table else None
-    rc = lib.gdrr_oracle_project(
-        *args, ctypes.c_int64(n_pix),
-        None if pix is None else pix.ctypes.data_as(_c_i32_p),
-        _dp(signal), _dp(li), None if tab is None else tab.ctypes.data_as(_c_i32_p),
-        ctypes.c_int(n_threads))
+    common = (*args, ctypes.c_int64(n_pix),
+              None if pix is None else pix.ctypes.data_as(_c_i32_p),
+              _dp(signal), _dp(li), None if tab is None else tab.ctypes.data_as(_c_i32_p))
+    if method == "siddon":
+        nseg = np.zeros(signal.shape, dtype=np.int32)
+        rc = lib.gdrr_oracle_project_siddon(*common, nseg.ctypes.data_as(_c_i32_p), ctypes.c_int(n_threads))
+        out = dict(signal=signal, line_integrals=li, ray_table=tab, n_segments=nseg)
+    elif method == "trilinear":
+        rc = lib.gdrr_oracle_project(*common, ctypes.c_int(n_threads))
+        out = dict(signal=signal, line_integrals=li, ray_table=tab)
+    else:
+        raise ValueError(f"unknown method {method!r}")
     if rc:
         raise ValueError("gdrr_oracle_project: invalid arguments")
-    return dict(signal=signal, line_integrals=li, ray_table=tab)
+    return out
 
 
 def project_literal(w, pixels, step=None, n_threads=0):
