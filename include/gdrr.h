@@ -72,14 +72,21 @@ enum {
  * carry a one-voxel replicated-edge pad, so clamp-to-edge costs no instruction.
  * BRICK and LINEAR hold, per voxel, one fp32 per material (rho at the voxel's
  * own material, 0 elsewhere; vector width 1, 2 or 4 floats), rho bit-exact.
- * PACKED_QUAD (the fast one) holds one 32-bit word per voxel -- fp32 rho rounded
- * to a 22-bit mantissa with the material index in the two freed bits when
- * n_materials > 1 (|stored - rho| <= 5 ulp = 3e-7 relative) -- as overlapping
- * 2x2 (x, y) quads, 16 bytes per voxel. */
+ * PACKED_QUAD (the fast one) holds one 32-bit word per voxel -- with more than
+ * one material, fp32 rho rounded to a 21-bit mantissa with the material index
+ * and a "pure cell" flag in the three freed bits (|stored - rho| <= 11 ulp =
+ * 1.3e-6 relative) -- as overlapping 2x2 (x, y) quads, 16 bytes per voxel. */
 enum {
     GDRR_LAYOUT_BRICK = 0,       /* 2x2x2-voxel bricks, x fastest inside a brick, bricks x fastest */
     GDRR_LAYOUT_LINEAR = 1,      /* plain [nz+2][ny+2][nx+2], x fastest */
-    GDRR_LAYOUT_PACKED_QUAD = 2  /* quads of packed words, 4x2 tiles per slab, slabs linear */
+    GDRR_LAYOUT_PACKED_QUAD = 2  /* quads of packed words, linear with bank-skewed strides */
+};
+
+/* How the line integrals of Eq. (1) are evaluated. */
+enum {
+    GDRR_METHOD_TRILINEAR = 0,   /* the paper's default: fixed-step midpoint rule on the tri-linear field */
+    GDRR_METHOD_SIDDON = 1       /* the paper's option: Siddon's exact radiological path through
+                                    homogeneous voxels, LI_m = sum_voxels rho [mat = m] |ray /\ voxel| */
 };
 
 #define GDRR_MAX_MATERIALS 4
@@ -184,6 +191,25 @@ GDRR_API int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_be
 GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
                       int proj_count, float* signal_host, float* signal_stage_dev,
                       int stage_proj, void* cuda_stream);
+
+/* Selects the line-integral method of the following gdrr_project calls on ctx
+ * (default GDRR_METHOD_TRILINEAR).  GDRR_METHOD_SIDDON ("Siddon's
+ * ray-tracing algorithm is also available in gDRR for primary signal
+ * calculation"): voxel (ix,iy,iz) is the homogeneous box [lo + i d, lo + (i+1) d)
+ * per axis, the path is the source->pixel segment clipped to the volume box,
+ * and every voxel contributes rho times the length of the ray inside it to the
+ * line integral of its material; the energy sum, the outputs and the ray table
+ * (which stays the midpoint table of the geometry) are unchanged.  A ray that
+ * lies IN a lattice plane belongs to either neighbour (a tie).  Works on every
+ * layout (on PACKED_QUAD it reads the first word of each quad).
+ * Errors: INVALID_ARG (unknown method). */
+GDRR_API int gdrr_set_method(gdrr_context* ctx, int method);
+
+/* Siddon traversal only: writes, per ray of the range, the number of voxel
+ * segments of positive length into n_segments_dev [proj_count][nv][nu] int32
+ * (0 for a miss).  Asynchronous on cuda_stream. */
+GDRR_API int gdrr_siddon_segments(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
+                         int proj_count, int32_t* n_segments_dev, void* cuda_stream);
 
 /* Ray setup only (step a1): writes the integer ray table and/or adds the
  * number of tri-linear samples sum(n) of the range to *n_samples_dev (a device

@@ -27,6 +27,8 @@ GDRR_ERR_UNSUPPORTED = -5
 GDRR_LAYOUT_BRICK = 0
 GDRR_LAYOUT_LINEAR = 1
 GDRR_LAYOUT_PACKED_QUAD = 2
+GDRR_METHOD_TRILINEAR = 0
+GDRR_METHOD_SIDDON = 1
 GDRR_MAX_MATERIALS = 4
 GDRR_MAX_ENERGIES = 512
 
@@ -35,6 +37,7 @@ EXPORTS = (
     "gdrr_volume_workspace_bytes", "gdrr_create_volume", "gdrr_create_volume_host",
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
+    "gdrr_set_method", "gdrr_siddon_segments",
 )
 
 
@@ -65,11 +68,17 @@ def _load():
         "gdrr_project": (i, [vp, vp, i, i, vp, vp, vp, vp]),
         "gdrr_project_host": (i, [vp, vp, i, i, vp, vp, i, vp]),
         "gdrr_ray_setup": (i, [vp, vp, i, i, vp, vp, vp]),
+        "gdrr_set_method": (i, [vp, i]),
+        "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
         "gdrr_kernel_launches": (ctypes.c_ulonglong, [vp]),
         "gdrr_version": (ctypes.c_char_p, []),
     }
     for name, (res, args) in sig.items():
-        fn = getattr(lib, name)          # AttributeError if the export is missing
+        try:
+            fn = getattr(lib, name)
+        except AttributeError as e:
+            raise ImportError(f"{path} does not export {name}: it is older than include/gdrr.h; rebuild it with "
+                              "`python paper_1204_6367_b200/build.py --force`") from e
         fn.restype = res
         fn.argtypes = args
     return lib
@@ -248,6 +257,15 @@ def gdrr_ray_setup(ctx, vol, proj_begin, proj_count, ray_table_dev=None, n_sampl
                                _dev(n_samples_dev, "int64", 1, "n_samples_dev"), _stream(stream)), ctx)
 
 
+def gdrr_set_method(ctx, method):
+    _check(_lib.gdrr_set_method(ctx, int(method)), ctx)
+
+
+def gdrr_siddon_segments(ctx, vol, proj_begin, proj_count, n_segments_dev, stream=None):
+    _check(_lib.gdrr_siddon_segments(ctx, vol, int(proj_begin), int(proj_count),
+                                     _dev(n_segments_dev, "int32", 0, "n_segments_dev"), _stream(stream)), ctx)
+
+
 def gdrr_kernel_launches(ctx):
     return int(_lib.gdrr_kernel_launches(ctx))
 
@@ -260,7 +278,8 @@ class Projector:
     """Context + volume + the torch tensors they borrow, built from a
     workload-like object (attributes as workloads.Workload)."""
 
-    def __init__(self, w, device=0, layout=GDRR_LAYOUT_PACKED_QUAD, from_host=False):
+    def __init__(self, w, device=0, layout=GDRR_LAYOUT_PACKED_QUAD, from_host=False,
+                 method=GDRR_METHOD_TRILINEAR):
         import torch
         self.torch = torch
         self.device = torch.device("cuda", device)
@@ -268,6 +287,7 @@ class Projector:
         self.ctx = gdrr_create_context(device)
         self.vol = None
         self.layout = layout
+        gdrr_set_method(self.ctx, method)
         gdrr_set_geometry(self.ctx, w.sad, w.sdd, w.theta, w.nu, w.nv, w.du, w.dv, w.u_off, w.v_off,
                           w.phis, w.step_mm)
         gdrr_set_spectrum(self.ctx, w.phi_weight, w.response, w.mu_hat, w.fluence_map, w.bowtie_mu,
@@ -324,6 +344,14 @@ class Projector:
             total = torch.zeros(1, dtype=torch.int64, device=self.device)
             gdrr_ray_setup(self.ctx, self.vol, proj_begin, n, None, total)
             return int(total.item())
+
+    def siddon_segments(self, proj_begin=0, proj_count=None):
+        torch, w = self.torch, self.w
+        n = w.n_proj - proj_begin if proj_count is None else proj_count
+        with torch.cuda.device(self.device):
+            out = torch.empty((n, w.nv, w.nu), dtype=torch.int32, device=self.device)
+            gdrr_siddon_segments(self.ctx, self.vol, proj_begin, n, out)
+        return out
 
     def kernel_launches(self):
         return gdrr_kernel_launches(self.ctx)

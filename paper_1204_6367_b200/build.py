@@ -1,7 +1,9 @@
 """Builds libgdrr_b200.so (the C-ABI library of include/gdrr.h) in-tree with nvcc
 for sm_100a.  nvcc cross-compiles without a GPU.
 
-    python -m paper_1204_6367_b200.build [--force] [--verbose]
+    python paper_1204_6367_b200/build.py [--force] [--verbose]
+
+(run as a file: importing the package first would load the library that is being replaced)
 """
 import os
 import shutil
@@ -12,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgdrr_b200.so")
-SOURCES = ["gdrr_api.cu", "project_fused.cu", "project_packed.cu", "volume_layout.cu"]
+SOURCES = ["gdrr_api.cu", "project_fused.cu", "project_packed.cu", "project_siddon.cu", "volume_layout.cu"]
 HEADERS = ["gdrr_internal.h", "ray_setup.cuh", "project_common.cuh", os.path.join(ROOT, "include", "gdrr.h")]
 
 NVCC_FLAGS = [

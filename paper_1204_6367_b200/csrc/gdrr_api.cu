@@ -39,6 +39,7 @@ struct gdrr_context {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
+    int method = GDRR_METHOD_TRILINEAR;
 };
 
 struct gdrr_volume {
@@ -196,6 +197,8 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     if (ctx->n_mat != vol->n_mat)
         return fail(ctx, GDRR_ERR_NOT_READY, "spectrum has %d materials, volume has %d", ctx->n_mat, vol->n_mat);
     P.v.vox = vol->vox;
+    P.v.nvox[0] = vol->nx; P.v.nvox[1] = vol->ny; P.v.nvox[2] = vol->nz;
+    P.seg_table = nullptr;
     if (vol->layout == GDRR_LAYOUT_BRICK) {
         P.v.stride_y = 8 * (vol->px / 2);
         P.v.stride_z = 8 * (vol->px / 2) * (vol->py / 2);
@@ -227,6 +230,7 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
 }
 
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
+    if (vol->ctx->method == GDRR_METHOD_SIDDON) return launch_project_siddon(P, vol->vw, vol->layout, s);
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);
 }
@@ -550,6 +554,30 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
     // later work on the caller's stream must not overtake the drains either
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gdrr_project_host");
+    return GDRR_OK;
+}
+
+int gdrr_set_method(gdrr_context* ctx, int method) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (method != GDRR_METHOD_TRILINEAR && method != GDRR_METHOD_SIDDON)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown method %d", method);
+    ctx->method = method;
+    return GDRR_OK;
+}
+
+int gdrr_siddon_segments(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                         int32_t* n_segments_dev, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!n_segments_dev) return fail(ctx, GDRR_ERR_INVALID_ARG, "n_segments_dev is NULL");
+    ProjectParams P;
+    int rc = fill_project(ctx, vol, proj_begin, proj_count, P);
+    if (rc) return rc;
+    P.signal = nullptr; P.li = nullptr; P.ray_table = nullptr; P.seg_table = n_segments_dev;
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaError_t e = launch_project_siddon(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "Siddon kernel launch");
+    ctx->launches += 1;
     return GDRR_OK;
 }
 

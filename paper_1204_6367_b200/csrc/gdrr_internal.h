@@ -33,6 +33,7 @@ struct VolumeParams {
     const void* vox;                // device, layout below
     const void* vox1;               // PACKED_QUAD: vox + one slab (its own parameter: one IMAD.WIDE per load)
     int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: elements per row (= 3 mod 8)
+    int nvox[3];                    // nx, ny, nz (Siddon traversal)
     int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab (= 4 mod 8)
 };
 
@@ -49,6 +50,7 @@ struct ProjectParams {
     float* signal;                  // [proj_count][nv][nu]
     float* li;                      // [proj_count][n_mat][nv][nu] or nullptr
     int32_t* ray_table;             // [proj_count][nv][nu][2] or nullptr
+    int32_t* seg_table;             // Siddon only: [proj_count][nv][nu] segments of positive length, or nullptr
 };
 
 struct IngestParams {
@@ -66,6 +68,7 @@ struct IngestParams {
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
+cudaError_t launch_project_siddon(const ProjectParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 

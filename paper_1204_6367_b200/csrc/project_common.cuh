@@ -56,15 +56,15 @@ __device__ __forceinline__ void index_line(const GeomParams& g, const Ray& r, do
     }
 }
 
-// Steps a5-a7: scale by dl, optional LI output, energy sum with the tables in
+// Steps a5-a7: scale the sums (by dl for the midpoint rule, by 1 for Siddon's lengths), optional LI output, energy sum with the tables in
 // shared memory (exp as ex2 of pre-scaled arguments), store.
 template <int VW>
 __device__ __forceinline__ void finish_pixel(const ProjectParams& P, const float4* s_mu,
                                              const float2* s_src, const float (&acc)[VW],
-                                             int pl, int i, int j) {
+                                             double scale, int pl, int i, int j) {
     float li[VW];
 #pragma unroll
-    for (int m = 0; m < VW; ++m) li[m] = (float)((double)acc[m] * P.g.step);
+    for (int m = 0; m < VW; ++m) li[m] = (float)((double)acc[m] * scale);
     if (P.li) {
         const size_t plane = (size_t)P.g.nv * P.g.nu;
         float* o = P.li + (size_t)pl * P.n_mat * plane + (size_t)j * P.g.nu + i;

@@ -132,7 +132,7 @@ gdrr_project_kernel(const ProjectParams P) {
         for (int m = 0; m < VW; ++m) acc[m] += part[m];
     }
 
-    finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
+    finish_pixel<VW>(P, s_mu, s_src, acc, P.g.step, pl, i, j);
 }
 
 // Ray setup alone: the integer ray table and/or the sample count sum(n).

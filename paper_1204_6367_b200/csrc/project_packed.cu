@@ -285,7 +285,7 @@ gdrr_project_packed_kernel(const ProjectParams P) {
         for (int m = 0; m < VW; ++m) acc[m] += A.part[m];
     }
 
-    if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, pl, i, j);
+    if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, P.g.step, pl, i, j);
 }
 
 template <int VW>

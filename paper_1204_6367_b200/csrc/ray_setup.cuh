@@ -15,6 +15,7 @@ struct Ray {
     double dir[3];      // unit direction source -> pixel centre
     double t_in, t_out; // parameter range inside the volume box
     int j0, n;          // first midpoint index, number of midpoints (0 = miss)
+    bool hit;           // the clipped segment [t_in, t_out] is not empty
 };
 
 __device__ __forceinline__ void ray_setup(const GeomParams& g, int p, int i, int j, Ray& r) {
@@ -56,6 +57,7 @@ __device__ __forceinline__ void ray_setup(const GeomParams& g, int p, int i, int
     }
     r.t_in = t_in;
     r.t_out = t_out;
+    r.hit = !miss && t_out > t_in;
 
     // midpoints t_k = (k + 1/2) dl laid from the source; count t_in <= t_k < t_out  [Q9]
     int j0 = 0, n = 0;

@@ -1,0 +1,140 @@
+"""GPU parity of GDRR_METHOD_SIDDON (exact radiological path) against the
+oracle's Siddon option on the same seeded inputs, through the C ABI.
+
+Bars: signal within 1e-4 relative per pixel, line integrals within 1e-4 relative plus the 1e-6
+floor, exactly 0 where the oracle has 0, the midpoint ray table (a property of the geometry, not of
+the method) bit-exact.  The number of voxel segments of positive length is unique only in exact
+arithmetic: where a ray passes within rounding of a lattice edge (near-ties, frequent for rays that
+run almost inside a lattice plane of these symmetric phantoms) a sliver of 1e-6 mm exists in fp64
+and not in fp32.  So the hit mask must be identical, and the counts must agree on all but a few
+percent of the rays, within a few percent per ray, and in total to 1e-3 (measured on C2: 0.5% of
+the rays differ, by at most 10 of ~280 segments)."""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from parity_util import check_line_integrals, check_ray_table, check_signal  # noqa: E402
+from test_oracle_pins import tiny_workload  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def gdrr():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    import paper_1204_6367_b200 as g
+    return g
+
+
+def check_segments(seg_gpu, seg_ref, what=""):
+    seg_gpu, seg_ref = np.asarray(seg_gpu, dtype=np.int64), np.asarray(seg_ref, dtype=np.int64)
+    assert seg_gpu.shape == seg_ref.shape
+    assert np.array_equal(seg_gpu == 0, seg_ref == 0), f"{what}: hit mask differs"
+    diff = np.abs(seg_gpu - seg_ref)
+    assert np.all(diff <= 4 + 0.05 * seg_ref), f"{what}: segment counts differ by up to {int(diff.max())}"
+    assert np.count_nonzero(diff) <= max(3, 0.03 * diff.size), f"{what}: {np.count_nonzero(diff)} rays differ"
+    assert abs(int(seg_gpu.sum()) - int(seg_ref.sum())) <= max(3, 1e-3 * int(seg_ref.sum())), what
+
+
+def compare_full_siddon(g, w, layout, what):
+    ref = oracle.project(w, method="siddon")
+    with g.Projector(w, layout=layout, method=g.GDRR_METHOD_SIDDON) as pr:
+        sig, li, tab = pr.project(want_li=True, want_table=True)
+        seg = pr.siddon_segments()
+    check_ray_table(tab.cpu().numpy(), ref["ray_table"], what)
+    rel_li, n_floor = check_line_integrals(li.cpu().numpy(), ref["line_integrals"], what)
+    worst = check_signal(sig.cpu().numpy(), ref["signal"], what)
+    check_segments(seg.cpu().numpy(), ref["n_segments"], what)
+    print(what, "signal", worst, "LI", rel_li, "floor pixels", n_floor)
+    return ref
+
+
+@pytest.mark.parametrize("layout", [0, 1, 2])
+@pytest.mark.parametrize("name", ["C0", "C1"])
+def test_siddon_full_image_small(gdrr, workloads_cache, name, layout):
+    compare_full_siddon(gdrr, workloads_cache(name), layout, f"siddon {name} layout {layout}")
+
+
+@pytest.mark.parametrize("phi_deg", [0.0, 37.0, 90.0, 225.0])
+def test_siddon_full_image_c2(gdrr, workloads_cache, phi_deg):
+    w = workloads_cache("C2").with_phis([math.radians(phi_deg)])
+    compare_full_siddon(gdrr, w, 2, f"siddon C2 phi {phi_deg}")
+
+
+def test_siddon_differs_from_trilinear_and_method_switches_back(gdrr, workloads_cache):
+    """The two methods integrate different fields (piecewise constant vs tri-linear): the images must
+    differ visibly on C1, and switching the method on one context must switch the result."""
+    w = workloads_cache("C1")
+    with gdrr.Projector(w) as pr:
+        tri, _, _ = pr.project()
+        gdrr.gdrr_set_method(pr.ctx, gdrr.GDRR_METHOD_SIDDON)
+        sid, _, _ = pr.project()
+        gdrr.gdrr_set_method(pr.ctx, gdrr.GDRR_METHOD_TRILINEAR)
+        tri2, _, _ = pr.project()
+        with pytest.raises(gdrr.GdrrError):
+            gdrr.gdrr_set_method(pr.ctx, 9)
+    assert torch.equal(tri, tri2)
+    rel = ((tri - sid).abs() / tri).max().item()
+    assert 1e-3 < rel < 0.5, rel
+    check_signal(sid.cpu().numpy(), oracle.project(w, method="siddon", want_li=False)["signal"], "switch")
+
+
+@pytest.mark.parametrize("layout", [0, 1, 2])
+@pytest.mark.parametrize("case", ["ragged", "odd_aniso_offcentre", "theta_offset", "three_materials", "one_voxel"])
+def test_siddon_edge_cases(gdrr, case, layout):
+    rng = np.random.default_rng(17)
+    kw = {}
+    if case == "ragged":                     # detector not a multiple of the 16 x 16 tile, volume dims odd
+        shape, n_mat, kw = (9, 13, 21), 2, dict(nu=37, nv=19, du=2.1, dv=2.3, phis=np.radians([11.0, 200.0]))
+    elif case == "odd_aniso_offcentre":
+        shape, n_mat, kw = (7, 12, 10), 1, dict(spacing=(1.3, 2.7, 3.1), centre=(12.0, -7.0, 4.0), nu=30, nv=22,
+                                                 phis=np.radians([63.0]))
+    elif case == "theta_offset":
+        shape, n_mat, kw = (10, 10, 10), 2, dict(theta=math.radians(8.0), nu=26, nv=18, phis=np.radians([100.0, 301.0]))
+    elif case == "three_materials":
+        shape, n_mat, kw = (12, 11, 10), 3, dict(nu=24, nv=20, phis=np.radians([45.0]))
+    else:
+        shape, n_mat, kw = (1, 1, 1), 1, dict(spacing=(20.0, 20.0, 20.0), nu=22, nv=18, phis=np.radians([30.0]))
+    rho = rng.uniform(0.0, 2.0, size=shape).astype(np.float32)
+    rho[rng.uniform(size=shape) < 0.2] = 0.0
+    mat = rng.integers(0, n_mat, size=shape).astype(np.uint8)
+    w = tiny_workload(rho, mat, n_materials=n_mat, mu_hat=rng.uniform(0.01, 0.03, size=(n_mat, 1)), **kw)
+    compare_full_siddon(gdrr, w, layout, f"siddon {case} layout {layout}")
+
+
+def test_siddon_axis_parallel_rays_and_all_miss(gdrr):
+    rng = np.random.default_rng(3)
+    rho = rng.uniform(0.5, 1.5, size=(5, 7, 9)).astype(np.float32)
+    # one pixel at u = v = 0: the ray is an axis (odd dims: through voxel centres, no lattice plane)
+    w = tiny_workload(rho, nu=1, nv=1, du=1.0, dv=1.0, phis=np.radians([0.0, 90.0, 180.0, 270.0]))
+    ref = compare_full_siddon(gdrr, w, 2, "siddon axis-parallel")
+    assert abs(ref["line_integrals"][0, 0, 0, 0] - 2.0 * float(rho[2, 3, :].astype(np.float64).sum())) < 1e-9
+    # a detector far off to the side: every ray misses the box -> flat field, zero segments
+    import copy
+    far = copy.copy(tiny_workload(rho, nu=8, nv=8, du=2.0, dv=2.0, phis=np.radians([20.0])))
+    far.u_off = 400.0
+    ref = compare_full_siddon(gdrr, far, 2, "siddon all-miss")
+    assert ref["n_segments"].max() == 0
+
+
+def test_siddon_c3_full_size_sampled(gdrr, workloads_cache):
+    """C3 in the launch configuration bench.py --method siddon times: sampled pixels of 6 projections."""
+    w = workloads_cache("C3")
+    n = w.n_proj
+    rng = np.random.default_rng(5)
+    with gdrr.Projector(w, method=gdrr.GDRR_METHOD_SIDDON) as pr:
+        for p in [0, n // 8, 37, n // 3, n // 2, n - 1]:
+            ii, jj = rng.integers(0, w.nu, 2000), rng.integers(0, w.nv, 2000)
+            ii[:5] = [0, w.nu - 1, 0, w.nu - 1, w.nu // 2]
+            jj[:5] = [0, 0, w.nv - 1, w.nv - 1, w.nv // 2]
+            ref = oracle.project(w, pixels=np.stack([np.full(2000, p), ii, jj], axis=1), method="siddon")
+            sig, li, _ = pr.project(proj_begin=p, proj_count=1, want_li=True)
+            seg = pr.siddon_segments(p, 1)
+            check_line_integrals(li[0].cpu().numpy()[:, jj, ii].T, ref["line_integrals"], f"siddon C3 p={p}")
+            check_signal(sig[0].cpu().numpy()[jj, ii], ref["signal"], f"siddon C3 p={p}")
+            check_segments(seg[0].cpu().numpy()[jj, ii], ref["n_segments"], f"siddon C3 p={p}")
