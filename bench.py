@@ -23,6 +23,8 @@ if ROOT not in sys.path:
 
 METRIC = "trilinear_samples_per_s"
 UNIT = "samples/s"
+METHODS = {"trilinear": ("trilinear_samples_per_s", "samples/s"),
+           "siddon": ("siddon_voxel_segments_per_s", "segments/s")}   # the paper's optional line integral
 SM_COUNT = 148
 L1_BYTES_PER_CLK = 128          # per SM, DESIGN.md "Roofline"
 
@@ -119,10 +121,14 @@ def oracle_sample(w, rows, projection):
 def time_oracle(w, pix):
     import oracle
     t0 = time.perf_counter()
-    out = oracle.project(w, pixels=pix, want_li=False)
+    out = oracle.project(w, pixels=pix, want_li=False, method=time_oracle.method)
     dt = time.perf_counter() - t0
     time_oracle.last_signal = out["signal"]                 # for the parity figure printed beside the timing
-    return int(out["ray_table"][:, 1].sum()), dt, oracle.n_threads_available()
+    units = out["n_segments"].sum() if time_oracle.method == "siddon" else out["ray_table"][:, 1].sum()
+    return int(units), dt, oracle.n_threads_available()
+
+
+time_oracle.method = "trilinear"
 
 
 def sized_oracle_sample(w, seconds):
@@ -203,10 +209,14 @@ def run_b200(args):
         w = w0.with_phis(np.full(per_gpu, np.deg2rad(args.angle_deg)))
     launch_proj = per_gpu if args.launch_proj <= 0 else min(args.launch_proj, per_gpu)
 
-    pr = g.Projector(w, device=local_rank, layout=args.layout)
+    pr = g.Projector(w, device=local_rank, layout=args.layout,
+                     method=g.GDRR_METHOD_SIDDON if args.method == "siddon" else g.GDRR_METHOD_TRILINEAR)
     signal = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32, device=dev)
     stream = torch.cuda.current_stream()
-    n_samples = pr.count_samples()
+    if args.method == "siddon":                            # units = voxel segments of positive length
+        n_samples = sum(int(pr.siddon_segments(b, min(32, per_gpu - b)).sum().item()) for b in range(0, per_gpu, 32))
+    else:
+        n_samples = pr.count_samples()
     ingest_launches_before = pr.kernel_launches()
 
     vw = 1 if w.n_materials == 1 else 2 if w.n_materials == 2 else 4
@@ -300,17 +310,21 @@ def run_b200(args):
 
     # ---- roofline of the dominant kernel (gdrr_project_kernel) ----------------------
     corner_bytes = 4 if args.layout == 2 else 4 * vw        # packed word, or one float per material
-    l1_bytes = 8 * corner_bytes * n_samples                 # 8 corners per sample
+    per_unit = 1 if args.method == "siddon" else 8          # one voxel per segment, 8 corners per sample
+    l1_bytes = per_unit * corner_bytes * n_samples
     l1_peak = SM_COUNT * L1_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9       # GB/s
     l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
     hbm_bytes = per_gpu * (vol_bytes + w.nu * w.nv * 4)
     hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
-    roofline = {"kernel": "gdrr_project_packed_kernel" if args.layout == 2 else "gdrr_project_kernel", "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
+    kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
+             "gdrr_project_packed_kernel" if args.layout == 2 else "gdrr_project_kernel")
+    roofline = {"kernel": kname, "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
                 "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
                 "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),
                 "peak_def": f"{SM_COUNT} SMs x {L1_BYTES_PER_CLK} B/clk x {peaks['sm_max_mhz']:.0f} MHz (max SM clock)",
-                "algorithmic": f"8 corners x {corner_bytes} B = {8 * corner_bytes} B per sample through L1",
+                "algorithmic": f"{per_unit} voxel value(s) x {corner_bytes} B = {per_unit * corner_bytes} B per "
+                               f"{'segment' if args.method == 'siddon' else 'sample'} through L1",
                 "samples_per_clk_per_sm": n_samples / (kernel_ms * 1e-3) / (SM_COUNT * peaks["sm_max_mhz"] * 1e6),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
@@ -327,7 +341,7 @@ def run_b200(args):
                "sample": f"{sample} ({n} samples)",
                "max_rel_err_of_b200_signal_on_sample": float(np.max(np.abs(got - ref) / ref))}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "method": args.method, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
@@ -349,6 +363,8 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--projections", type=int, default=0, help="projections per GPU (0 = the workload's)")
     ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
+    ap.add_argument("--method", default="trilinear", choices=sorted(METHODS),
+                    help="line integral: the paper's default tri-linear midpoint rule, or its Siddon option")
     ap.add_argument("--angle-deg", type=float, default=None,
                     help="profiling aid: all projections at this one gantry angle instead of an evenly spaced scan")
     ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")
@@ -359,6 +375,9 @@ def main():
     ap.add_argument("--ncu-dram-bytes", type=float, default=0.0,
                     help="dram bytes per launch from the committed ncu capture (profiles/)")
     args = ap.parse_args()
+    global METRIC, UNIT
+    METRIC, UNIT = METHODS[args.method]
+    time_oracle.method = args.method
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -49,11 +49,42 @@ __device__ __forceinline__ int siddon_axis_offset(int i, int stride) {
     return i * stride;
 }
 
-// LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed quad (first word of a quad)
+// len x voxel value into the per-material sums.  Exact layouts: one FMA per material.  Packed word:
+// a running sum of the current material, routed when the material changes.
+template <int VW, int LAYOUT, class VT>
+__device__ __forceinline__ void accumulate_voxel(const VT& v, float len, float (&part)[VW], float& cur, unsigned& curm) {
+    if constexpr (LAYOUT == 2) {
+        if (VW > 1) {
+            const unsigned m = v & 3u;
+            if (m != curm) {
+                add_routed_s<VW>(part, (int)curm, cur);
+                cur = 0.f;
+                curm = m;
+            }
+        }
+        cur = fmaf(len, __uint_as_float(v), cur);
+    } else {
+        add_len(part, len, v);
+    }
+}
+
+// One voxel value: the exact layouts hold VW floats, the packed layout one tagged word.
+template <int VW, int LAYOUT> struct SiddonVoxel { using T = typename SVox<VW>::T; };
+template <int VW> struct SiddonVoxel<VW, 2> { using T = unsigned; };
+
 template <int VW, int LAYOUT>
+__device__ __forceinline__ typename SiddonVoxel<VW, LAYOUT>::T load_voxel(const void* vox, int off) {
+    using T = typename SiddonVoxel<VW, LAYOUT>::T;
+    if (LAYOUT == 2) return __ldg(reinterpret_cast<const T*>(vox) + 4 * (size_t)off);     // first word of the quad
+    return __ldg(reinterpret_cast<const T*>(vox) + off);
+}
+
+// LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed quad (first word of a quad)
+// COUNT: also count the segments of positive length (gdrr_siddon_segments)
+template <int VW, int LAYOUT, bool COUNT>
 __global__ void __launch_bounds__(kThreads)
 gdrr_project_siddon_kernel(const ProjectParams P) {
-    using V = typename SVox<VW>::T;
+    using VT = typename SiddonVoxel<VW, LAYOUT>::T;
     float4* s_mu;
     float2* s_src;
     load_tables(P, s_mu, s_src);
@@ -73,10 +104,9 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
     for (int m = 0; m < VW; ++m) acc[m] = 0.f;
     int n_seg = 0;
 
-    const double chord = r.t_out - r.t_in;
     if (r.hit) {
-        // ---- set-up of the traversal (fp64): voxel at the entry point, plane counters, parameters
-        int idx[3], stp[3], left[3];     // voxel index, +-1, planes still to cross before leaving the box
+        // ---- set-up of the traversal (fp64): voxel at the entry point, parameters of the next planes
+        int idx[3], stp[3];
         float t0[3], dt[3];              // parameter (relative to t_in) of the next plane, and per plane
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
@@ -87,88 +117,67 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
             idx[a] = v;
             if (r.dir[a] > 0.0) {
                 stp[a] = 1;
-                left[a] = N - v;
                 t0[a] = (float)((P.g.lo[a] + (double)(v + 1) * P.g.d[a] - r.S[a]) / r.dir[a] - r.t_in);
                 dt[a] = (float)(P.g.d[a] / r.dir[a]);
             } else if (r.dir[a] < 0.0) {
                 stp[a] = -1;
-                left[a] = v + 1;
                 t0[a] = (float)((P.g.lo[a] + (double)v * P.g.d[a] - r.S[a]) / r.dir[a] - r.t_in);
                 dt[a] = (float)(-P.g.d[a] / r.dir[a]);
             } else {
                 stp[a] = 0;
-                left[a] = 0x7fffffff;
                 t0[a] = 3.0e38f;
                 dt[a] = 0.f;
             }
         }
-        const float t_end = (float)chord;
+        const float t_end = (float)(r.t_out - r.t_in);
+        // The plane through which the ray leaves the box has the parameter t_end up to ~3 ulp (t0, dt and
+        // t_end are rounded separately): a crossing within 16 ulp of the end IS the end, so the walk never
+        // steps out of the lattice; the sliver it may drop is < 5e-4 mm of the last voxel.
+        const float t_stop = t_end * (1.f - 16.f * 5.96e-8f);
         constexpr int sx = (LAYOUT == 0) ? 8 : 1;
         const int sy = P.v.stride_y, sz = P.v.stride_z;
-        // element offsets of the padded voxel (idx + 1)
-        int ox = siddon_axis_offset<LAYOUT, 0>(idx[0] + 1, sx);
-        int oy = siddon_axis_offset<LAYOUT, 1>(idx[1] + 1, sy);
-        int oz = siddon_axis_offset<LAYOUT, 2>(idx[2] + 1, sz);
-        int kx = 0, ky = 0, kz = 0;                      // planes crossed so far per axis
+        int off = siddon_axis_offset<LAYOUT, 0>(idx[0] + 1, sx) + siddon_axis_offset<LAYOUT, 1>(idx[1] + 1, sy) +
+                  siddon_axis_offset<LAYOUT, 2>(idx[2] + 1, sz);
+        // linear element orders: stepping one voxel along an axis adds a constant to the element offset
+        const int dox = stp[0] * sx, doy = stp[1] * sy, doz = stp[2] * sz;
+        float kx = 0.f, ky = 0.f, kz = 0.f;              // planes crossed so far per axis (exact in fp32)
         float tx = t0[0], ty = t0[1], tz = t0[2];
         float t = 0.f;
         unsigned curm = 0;
         float cur = 0.f;
-        bool inside = true;
 
-        while (inside) {
+        // the voxel of segment s + 1 is requested before segment s is accumulated
+        VT v = load_voxel<VW, LAYOUT>(P.v.vox, off);
+        bool more = true;
+        while (more) {
             float part[VW];
 #pragma unroll
             for (int m = 0; m < VW; ++m) part[m] = 0.f;
-            for (int s = 0; s < kMaxChunk && inside; ++s) {
-                // the voxel the ray is in, and where it leaves it
-                const float tn = fminf(fminf(tx, ty), fminf(tz, t_end));
+            for (int s = 0; s < kMaxChunk && more; ++s) {
+                const float tn = fminf(fminf(tx, ty), fminf(tz, t_end));    // where the ray leaves this voxel
                 const float len = tn - t;
-                if (LAYOUT == 2) {
-                    const unsigned w = __ldg(reinterpret_cast<const unsigned*>(P.v.vox) + 4 * (size_t)(oz + oy + ox));
-                    if (len > 0.f) {
-                        ++n_seg;
-                        if (VW == 1) {
-                            cur = fmaf(len, __uint_as_float(w), cur);
-                        } else {
-                            const unsigned m = w & 3u;
-                            if (m != curm) {
-                                add_routed_s<VW>(part, (int)curm, cur);
-                                cur = 0.f;
-                                curm = m;
-                            }
-                            cur = fmaf(len, __uint_as_float(w), cur);
-                        }
-                    }
-                } else {
-                    const V v = __ldg(reinterpret_cast<const V*>(P.v.vox) + (oz + oy + ox));
-                    if (len > 0.f) {
-                        ++n_seg;
-                        add_len(part, len, v);
-                    }
-                }
                 t = fmaxf(tn, t);
-                // step into the next voxel across the plane that was met (x before y before z at ties)
-                if (tn >= t_end) {
-                    inside = false;
-                } else if (tx <= ty && tx <= tz) {
-                    ++kx;
-                    idx[0] += stp[0];
-                    ox = siddon_axis_offset<LAYOUT, 0>(idx[0] + 1, sx);
-                    tx = fmaf((float)kx, dt[0], t0[0]);
-                    inside = kx < left[0];
-                } else if (ty <= tz) {
-                    ++ky;
-                    idx[1] += stp[1];
-                    oy = siddon_axis_offset<LAYOUT, 1>(idx[1] + 1, sy);
-                    ty = fmaf((float)ky, dt[1], t0[1]);
-                    inside = ky < left[1];
+                more = tn < t_stop;
+                // cross the plane that was met (x before y before z at ties), branch-free
+                const bool bx = tx <= ty && tx <= tz;
+                const bool by = !bx && ty <= tz;
+                if (LAYOUT == 0) {
+                    idx[0] += bx ? stp[0] : 0;
+                    idx[1] += by ? stp[1] : 0;
+                    idx[2] += (bx || by) ? 0 : stp[2];
+                    off = siddon_axis_offset<0, 0>(idx[0] + 1, sx) + siddon_axis_offset<0, 1>(idx[1] + 1, sy) +
+                          siddon_axis_offset<0, 2>(idx[2] + 1, sz);
                 } else {
-                    ++kz;
-                    idx[2] += stp[2];
-                    oz = siddon_axis_offset<LAYOUT, 2>(idx[2] + 1, sz);
-                    tz = fmaf((float)kz, dt[2], t0[2]);
-                    inside = kz < left[2];
+                    off += bx ? dox : (by ? doy : doz);
+                }
+                if (bx) { kx += 1.f; tx = fmaf(kx, dt[0], t0[0]); }
+                else if (by) { ky += 1.f; ty = fmaf(ky, dt[1], t0[1]); }
+                else { kz += 1.f; tz = fmaf(kz, dt[2], t0[2]); }
+                const VT cv = v;
+                if (more) v = load_voxel<VW, LAYOUT>(P.v.vox, off);
+                if (len > 0.f) {
+                    if (COUNT) ++n_seg;
+                    accumulate_voxel<VW, LAYOUT>(cv, len, part, cur, curm);
                 }
             }
             if (LAYOUT == 2) {
@@ -180,16 +189,22 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
         }
     }
 
-    if (P.seg_table) P.seg_table[pix] = n_seg;
+    if (COUNT && P.seg_table) P.seg_table[pix] = n_seg;
     if (P.signal) finish_pixel<VW>(P, s_mu, s_src, acc, 1.0, pl, i, j);
+}
+
+template <int VW, int LAYOUT, bool COUNT>
+static cudaError_t launch_siddon_c(const ProjectParams& p, cudaStream_t s) {
+    dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
+    const size_t smem = (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
+    gdrr_project_siddon_kernel<VW, LAYOUT, COUNT><<<grid, kThreads, smem, s>>>(p);
+    return cudaGetLastError();
 }
 
 template <int VW, int LAYOUT>
 static cudaError_t launch_siddon_t(const ProjectParams& p, cudaStream_t s) {
-    dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
-    const size_t smem = (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
-    gdrr_project_siddon_kernel<VW, LAYOUT><<<grid, kThreads, smem, s>>>(p);
-    return cudaGetLastError();
+    if (p.seg_table) return launch_siddon_c<VW, LAYOUT, true>(p, s);
+    return launch_siddon_c<VW, LAYOUT, false>(p, s);
 }
 
 cudaError_t launch_project_siddon(const ProjectParams& p, int vw, int layout, cudaStream_t s) {
