@@ -89,6 +89,14 @@ enum {
                                     homogeneous voxels, LI_m = sum_voxels rho [mat = m] |ray /\ voxel| */
 };
 
+/* Which kernel samples a PACKED_QUAD volume with the tri-linear method.  Both give the same
+ * numbers to rounding order (the staged one sums in chunks of 16 samples, the gather one of 32). */
+enum {
+    GDRR_SAMPLER_AUTO = 0,     /* STAGED when the volume's tensor map could be made, else GATHER */
+    GDRR_SAMPLER_GATHER = 1,   /* quads gathered from global memory through L1 */
+    GDRR_SAMPLER_STAGED = 2    /* quads of a CTA's beam staged through shared memory by TMA */
+};
+
 #define GDRR_MAX_MATERIALS 4
 #define GDRR_MAX_ENERGIES 512
 
@@ -204,6 +212,10 @@ GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int pr
  * layout (on PACKED_QUAD it reads the first word of each quad).
  * Errors: INVALID_ARG (unknown method). */
 GDRR_API int gdrr_set_method(gdrr_context* ctx, int method);
+
+/* Selects the sampling kernel for PACKED_QUAD volumes (default GDRR_SAMPLER_AUTO).
+ * Errors: INVALID_ARG (unknown value). */
+GDRR_API int gdrr_set_sampler(gdrr_context* ctx, int sampler);
 
 /* Siddon traversal only: writes, per ray of the range, the number of voxel
  * segments of positive length into n_segments_dev [proj_count][nv][nu] int32

@@ -27,6 +27,9 @@ GDRR_ERR_UNSUPPORTED = -5
 GDRR_LAYOUT_BRICK = 0
 GDRR_LAYOUT_LINEAR = 1
 GDRR_LAYOUT_PACKED_QUAD = 2
+GDRR_SAMPLER_AUTO = 0
+GDRR_SAMPLER_GATHER = 1
+GDRR_SAMPLER_STAGED = 2
 GDRR_METHOD_TRILINEAR = 0
 GDRR_METHOD_SIDDON = 1
 GDRR_MAX_MATERIALS = 4
@@ -37,7 +40,7 @@ EXPORTS = (
     "gdrr_volume_workspace_bytes", "gdrr_create_volume", "gdrr_create_volume_host",
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
-    "gdrr_set_method", "gdrr_siddon_segments",
+    "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler",
 )
 
 
@@ -69,6 +72,7 @@ def _load():
         "gdrr_project_host": (i, [vp, vp, i, i, vp, vp, i, vp]),
         "gdrr_ray_setup": (i, [vp, vp, i, i, vp, vp, vp]),
         "gdrr_set_method": (i, [vp, i]),
+        "gdrr_set_sampler": (i, [vp, i]),
         "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
         "gdrr_kernel_launches": (ctypes.c_ulonglong, [vp]),
         "gdrr_version": (ctypes.c_char_p, []),
@@ -261,6 +265,10 @@ def gdrr_set_method(ctx, method):
     _check(_lib.gdrr_set_method(ctx, int(method)), ctx)
 
 
+def gdrr_set_sampler(ctx, sampler):
+    _check(_lib.gdrr_set_sampler(ctx, int(sampler)), ctx)
+
+
 def gdrr_siddon_segments(ctx, vol, proj_begin, proj_count, n_segments_dev, stream=None):
     _check(_lib.gdrr_siddon_segments(ctx, vol, int(proj_begin), int(proj_count),
                                      _dev(n_segments_dev, "int32", 0, "n_segments_dev"), _stream(stream)), ctx)
@@ -279,7 +287,7 @@ class Projector:
     workload-like object (attributes as workloads.Workload)."""
 
     def __init__(self, w, device=0, layout=GDRR_LAYOUT_PACKED_QUAD, from_host=False,
-                 method=GDRR_METHOD_TRILINEAR):
+                 method=GDRR_METHOD_TRILINEAR, sampler=GDRR_SAMPLER_AUTO):
         import torch
         self.torch = torch
         self.device = torch.device("cuda", device)
@@ -288,6 +296,7 @@ class Projector:
         self.vol = None
         self.layout = layout
         gdrr_set_method(self.ctx, method)
+        gdrr_set_sampler(self.ctx, sampler)
         gdrr_set_geometry(self.ctx, w.sad, w.sdd, w.theta, w.nu, w.nv, w.du, w.dv, w.u_off, w.v_off,
                           w.phis, w.step_mm)
         gdrr_set_spectrum(self.ctx, w.phi_weight, w.response, w.mu_hat, w.fluence_map, w.bowtie_mu,

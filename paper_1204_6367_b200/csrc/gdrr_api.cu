@@ -2,6 +2,8 @@
 // small context-owned device tables, and kernel launches.  No arithmetic of the
 // method happens here except what the header says is done on the host: cos/sin
 // of the gantry angles (given to the kernels as data) and table pre-scaling.
+#include <cuda.h>
+
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
@@ -40,6 +42,7 @@ struct gdrr_context {
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
     int method = GDRR_METHOD_TRILINEAR;
+    int sampler = GDRR_SAMPLER_AUTO;
 };
 
 struct gdrr_volume {
@@ -49,6 +52,8 @@ struct gdrr_volume {
     double d[3], c[3];
     int n_mat, vw, layout;
     int sy, sz;                 // PACKED_QUAD: element strides
+    bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
+    alignas(64) CUtensorMap tmap;
 };
 
 static thread_local std::string g_create_err;
@@ -229,8 +234,35 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     return GDRR_OK;
 }
 
+// Tensor map of the packed-quad volume for project_staged.cu: a 3-D tensor of 32-bit words
+// (4 px words along x, py rows of pitch 16 sy bytes, pz slabs of pitch 16 sz bytes), box
+// 56 words x 14 rows x 11 slabs.  The driver entry point is looked up at run time, so the
+// library still links cudart only.  Returns false if the driver cannot make it.
+bool make_tensor_map(gdrr_volume* v) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t dims[3] = {4ull * (cuuint64_t)v->px, (cuuint64_t)v->py, (cuuint64_t)v->pz};
+    const cuuint64_t strides[2] = {16ull * (cuuint64_t)v->sy, 16ull * (cuuint64_t)v->sz};      // bytes, dims 1 and 2
+    const cuuint32_t box[3] = {56u, 14u, 11u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    CUresult r = ((encode_fn)fn)(&v->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, v->vox, dims, strides, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
     if (vol->ctx->method == GDRR_METHOD_SIDDON) return launch_project_siddon(P, vol->vw, vol->layout, s);
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && vol->ctx->sampler != GDRR_SAMPLER_GATHER)
+        return launch_project_staged(P, vol->vw, &vol->tmap, s);
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);
 }
@@ -343,6 +375,7 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     for (int a = 0; a < 3; ++a) v->c[a] = centre_mm ? centre_mm[a] : 0.0;
     v->n_mat = n_materials; v->vw = vw; v->layout = layout;
     v->sy = ip.sy; v->sz = ip.sz;
+    v->has_tmap = layout == GDRR_LAYOUT_PACKED_QUAD && make_tensor_map(v);
     *out = v;
     return GDRR_OK;
 }
@@ -562,6 +595,14 @@ int gdrr_set_method(gdrr_context* ctx, int method) {
     if (method != GDRR_METHOD_TRILINEAR && method != GDRR_METHOD_SIDDON)
         return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown method %d", method);
     ctx->method = method;
+    return GDRR_OK;
+}
+
+int gdrr_set_sampler(gdrr_context* ctx, int sampler) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (sampler != GDRR_SAMPLER_AUTO && sampler != GDRR_SAMPLER_GATHER && sampler != GDRR_SAMPLER_STAGED)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown sampler %d", sampler);
+    ctx->sampler = sampler;
     return GDRR_OK;
 }
 

@@ -28,174 +28,9 @@
 // The words are used as floats as they are (|stored - rho| <= 11 ulp, DESIGN.md
 // Q24); the library is compiled with -ftz=true so that rho = 0 tagged with a
 // material (a denormal bit pattern) contributes exactly 0.
-#include "project_common.cuh"
+#include "packed_sampler.cuh"
 
 namespace gdrr {
-
-template <int VW>
-__device__ __forceinline__ void add_routed(float (&part)[VW], int m, float v) {
-#pragma unroll
-    for (int k = 0; k < VW; ++k) part[k] += (m == k) ? v : 0.f;
-}
-
-__device__ __forceinline__ float lerp(float a, float b, float t) { return fmaf(t, b - a, a); }
-
-// Packed fp32 pairs (sm_100 FADD2 / FFMA2: two fp32 lanes per instruction, same rounding as the
-// scalar forms; .ftz as the rest of the library).
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(unsigned lo, unsigned hi) {
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
-    return r;
-}
-__device__ __forceinline__ f32x2 bcast2(float v) {
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %1};" : "=l"(r) : "f"(v));
-    return r;
-}
-__device__ __forceinline__ f32x2 lerp2(f32x2 a, f32x2 b, f32x2 t) {       // a + t (b - a), per lane
-    f32x2 d, r;
-    asm("sub.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(b), "l"(a));
-    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(t), "l"(d), "l"(a));
-    return r;
-}
-// Tri-linear blend of one cell.  Words of a quad: (x0y0, x0y1, x1y0, x1y1), so that the two
-// x-lerps of a slab are one packed lerp between its register pairs, the two z-lerps another.
-__device__ __forceinline__ float blend_cell(const uint4& a, const uint4& c, float fx, float fy, float fz) {
-    const f32x2 tx = bcast2(fx), tz = bcast2(fz);
-    const f32x2 va = lerp2(pack2(a.x, a.y), pack2(a.z, a.w), tx);       // slab iz:     (y0, y1) at x
-    const f32x2 vc = lerp2(pack2(c.x, c.y), pack2(c.z, c.w), tx);       // slab iz + 1
-    const f32x2 v = lerp2(va, vc, tz);                                  // (y0, y1) at (x, z)
-    float y0, y1;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(y0), "=f"(y1) : "l"(v));
-    return lerp(y0, y1, fy);
-}
-
-// (q & mask) | one in a single LOP3; mask and one arrive as kernel parameters so
-// that they live in registers instead of being split into two immediate ops.
-__device__ __forceinline__ float frac_float(int q, unsigned mask, unsigned one) {
-    unsigned o;
-    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(o) : "r"(q), "r"(mask), "r"(one));
-    return __uint_as_float(o) - 1.f;
-}
-
-// thread -> pixel: a warp is 4 (u) x 8 (v) pixels, so that a load phase (8 consecutive lanes) is a
-// compact 4 x 2 patch of rays; the CTA's 16 x 16 tile is 4 x 2 warps.
-__device__ __forceinline__ void thread_pixel_map(int& i, int& j) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    i = blockIdx.x * kTileU + (warp & 3) * 4 + (lane & 3);
-    j = blockIdx.y * kTileV + (warp >> 2) * 8 + (lane >> 2);
-}
-
-// Element index of cell (cx, cy, cz): linear, strides sy = 3 and sz = 4 (mod 8).
-__device__ __forceinline__ int elem_index(int cx, int cy, int cz, int sy, int sz) {
-    return cz * sz + cy * sy + cx;
-}
-
-// UNI: every lane of the warp is here (unpredicated chunk): vote, so that the common case "all lanes
-// in a pure cell of their running material" is a warp-uniform branch without reconvergence overhead.
-template <int VW, bool UNI>
-__device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, float fx, float fy, float fz,
-                                             float& cur, unsigned& curm4, float (&part)[VW]) {
-    bool fast = true;
-    if (VW > 1) fast = (a.x & 7u) == curm4;        // pure cell of the running material
-    if (VW > 1 && UNI) {
-        if (__all_sync(0xffffffffu, fast)) {
-            cur += blend_cell(a, c, fx, fy, fz);
-            return;
-        }
-    }
-    if (fast) {
-        cur += blend_cell(a, c, fx, fy, fz);
-    } else {
-        // mixed cell, or a pure cell of another material: route every weighted corner
-        const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
-        const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
-        // w<y><z>; words (x0y0, x0y1, x1y0, x1y1)
-        add_routed<VW>(part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
-        add_routed<VW>(part, (int)(a.y & 3u), gx * w10 * __uint_as_float(a.y));
-        add_routed<VW>(part, (int)(a.z & 3u), fx * w00 * __uint_as_float(a.z));
-        add_routed<VW>(part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
-        add_routed<VW>(part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
-        add_routed<VW>(part, (int)(c.y & 3u), gx * w11 * __uint_as_float(c.y));
-        add_routed<VW>(part, (int)(c.z & 3u), fx * w01 * __uint_as_float(c.z));
-        add_routed<VW>(part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
-        // the running sum follows the material the ray is now in
-        const unsigned m4 = (c.w & 3u) | 4u;
-        if (m4 != curm4) {
-            add_routed<VW>(part, (int)(curm4 & 3u), cur);
-            cur = 0.f;
-            curm4 = m4;
-        }
-    }
-}
-
-// element of the sample at in-chunk fixed-point position q (idx0 = element of the chunk's base cell)
-__device__ __forceinline__ int sample_index(int idx0, int qx, int qy, int qz, int sy, int sz) {
-    return idx0 + (qz >> kFracBits) * sz + (qy >> kFracBits) * sy + (qx >> kFracBits);
-}
-
-// State of one ray while it is sampled.
-template <int VW>
-struct RayAcc {
-    float part[VW];     // per-material partial sums of the current chunk
-    float cur;          // running sum of pure cells of material curm4 & 3
-    unsigned curm4;     // 4 | material
-};
-
-struct Sampler {
-    const uint4* __restrict__ vol0;     // slab iz
-    const uint4* __restrict__ vol1;     // slab iz + 1
-    int sy, sz;
-    int dqx, dqy, dqz;
-    unsigned fmask, fone;
-};
-
-// `cnt` consecutive samples of a chunk.  PRED = false: every lane of the warp owns all of
-// them and cnt is even (the common case); PRED = true: sample s is this ray's iff
-// rel + s < un (first and last chunk of the warp).  Two register buffers: the loads of
-// sample s + 1 are in flight while sample s is blended.
-template <int VW, bool PRED>
-__device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, int cnt, unsigned rel, unsigned un,
-                                          RayAcc<VW>& A) {
-    int qx = b.qx, qy = b.qy, qz = b.qz;
-    const int idx0 = elem_index(b.cx, b.cy, b.cz, S.sy, S.sz);
-    uint4 a0 = make_uint4(0, 0, 0, 0), c0 = a0, a1 = a0, c1 = a0;
-    bool act0 = !PRED || rel < un;
-    if (act0) {
-        const int idx = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
-        a0 = __ldg(S.vol0 + idx);
-        c0 = __ldg(S.vol1 + idx);
-    }
-    for (int s = 0; s < cnt; s += 2) {
-        float fx = frac_float(qx, S.fmask, S.fone);
-        float fy = frac_float(qy, S.fmask, S.fone);
-        float fz = frac_float(qz, S.fmask, S.fone);
-        qx += S.dqx; qy += S.dqy; qz += S.dqz;
-        const bool more = !PRED || s + 1 < cnt;                  // warp-uniform
-        const bool act1 = more && (!PRED || rel + 1u < un);
-        if (act1) {
-            const int idx = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
-            a1 = __ldg(S.vol0 + idx);
-            c1 = __ldg(S.vol1 + idx);
-        }
-        if (act0) blend_sample<VW, !PRED>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
-        if (more) {
-            fx = frac_float(qx, S.fmask, S.fone);
-            fy = frac_float(qy, S.fmask, S.fone);
-            fz = frac_float(qz, S.fmask, S.fone);
-            qx += S.dqx; qy += S.dqy; qz += S.dqz;
-            rel += 2u;
-            act0 = (s + 2 < cnt) && (!PRED || rel < un);
-            if (act0) {
-                const int idx = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
-                a0 = __ldg(S.vol0 + idx);
-                c0 = __ldg(S.vol1 + idx);
-            }
-            if (act1) blend_sample<VW, !PRED>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
-        }
-    }
-}
 
 template <int VW>
 __global__ void __launch_bounds__(kThreads, 4)

@@ -1,0 +1,306 @@
+// Steps a1-a7 fused, PACKED-QUAD layout, quads STAGED THROUGH SHARED MEMORY BY TMA.
+//
+// Why.  The gather kernel (project_packed.cu) saturates the L1 data pipe: a 16-byte warp-wide
+// load costs 6.7 wavefronts instead of 4, because 1.3 of its sectors miss L1 (every quad is
+// first touched once per CTA beam, and each missed sector is served by a wavefront of its own)
+// and because of bank-group conflicts (profiles/r01_packed_kernel_ncu.md).  Here the quads a
+// CTA's 16 x 16 beam crosses during kStageK consecutive interval indices are fetched ONCE, as
+// one box of the device volume, by a bulk tensor copy (cp.async.bulk.tensor, TMA) straight
+// into shared memory, double buffered; the sampler then reads shared memory, where a load
+// never misses and the only cost above 4 wavefronts is bank conflicts.
+//
+// The box.  Intervals are laid from the source, so all rays of the CTA are at the same
+// interval index k and a chunk of kStageK indices is a thin curved slab of the beam.  Per
+// chunk every thread contributes the cells of its first and last sample of the chunk (the
+// cells in between are bracketed by them: positions are linear in k) to a CTA-wide bounding
+// box; thread 0 issues the copy of that box for chunk c + 1 while chunk c is sampled.  The box
+// has a fixed shape (kBX x kBY x kBZ quads: a tensor map fixes its box); a chunk whose
+// bounding box does not fit (other geometries) is sampled from global memory by the gather
+// path's own routine, so the result never depends on the staging.
+// Row pitch kBX = 14 = 6 (mod 8) and slab pitch kBX kBY = 196 = 4 (mod 8): neighbouring quads
+// fall in different 16-byte bank groups in every direction (profiles/r01_l1_model.md).
+#include <cuda.h>
+
+#include "packed_sampler.cuh"
+
+namespace gdrr {
+
+constexpr int kStageK = 16;                       // interval indices per staged chunk
+constexpr int kBX = 14, kBY = 14, kBZ = 11;       // box, in quads
+constexpr int kBoxElems = kBX * kBY * kBZ;        // 2156 quads = 34,496 B
+constexpr int kStageElems = 2160;                 // stage pitch: 34,560 B, a multiple of 128
+constexpr unsigned kBoxBytes = kBoxElems * 16u;
+
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+// box of the 3-D tensor (words along x, rows, slabs) at (c0, c1, c2) -> shared memory, completes on `bar`
+__device__ __forceinline__ void tma_load_box(void* dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                             unsigned long long* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(smem_addr(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_addr(bar)) : "memory");
+}
+
+// The quads of the staged boxes (2 stages), then the spectrum tables.
+extern __shared__ __align__(128) uint4 s_box[];
+
+// `cnt` consecutive samples of a chunk out of the staged box: as run_chunk (packed_sampler.cuh),
+// the element index is relative to the box and both slabs of a cell are read with one address.
+template <int VW, bool PRED>
+__device__ __forceinline__ void run_chunk_staged(const Sampler& S, int qx, int qy, int qz, int idx0, int cnt,
+                                                 unsigned rel, unsigned un, RayAcc<VW>& A) {
+    uint4 a0 = make_uint4(0, 0, 0, 0), c0 = a0, a1 = a0, c1 = a0;
+    bool act0 = !PRED || rel < un;
+    if (act0) {
+        const int idx = sample_index(idx0, qx, qy, qz, kBX, kBX * kBY);
+        a0 = s_box[idx];
+        c0 = s_box[idx + kBX * kBY];
+    }
+    for (int s = 0; s < cnt; s += 2) {
+        float fx = frac_float(qx, S.fmask, S.fone);
+        float fy = frac_float(qy, S.fmask, S.fone);
+        float fz = frac_float(qz, S.fmask, S.fone);
+        qx += S.dqx; qy += S.dqy; qz += S.dqz;
+        const bool more = !PRED || s + 1 < cnt;
+        const bool act1 = more && (!PRED || rel + 1u < un);
+        if (act1) {
+            const int idx = sample_index(idx0, qx, qy, qz, kBX, kBX * kBY);
+            a1 = s_box[idx];
+            c1 = s_box[idx + kBX * kBY];
+        }
+        if (act0) blend_sample<VW, !PRED>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
+        if (more) {
+            fx = frac_float(qx, S.fmask, S.fone);
+            fy = frac_float(qy, S.fmask, S.fone);
+            fz = frac_float(qz, S.fmask, S.fone);
+            qx += S.dqx; qy += S.dqy; qz += S.dqz;
+            rel += 2u;
+            act0 = (s + 2 < cnt) && (!PRED || rel < un);
+            if (act0) {
+                const int idx = sample_index(idx0, qx, qy, qz, kBX, kBX * kBY);
+                a0 = s_box[idx];
+                c0 = s_box[idx + kBX * kBY];
+            }
+            if (act1) blend_sample<VW, !PRED>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
+        }
+    }
+}
+
+// CTA-shared bookkeeping of the staging pipeline
+struct StageCtl {
+    unsigned long long bar[2];     // "box of stage s has landed"
+    int bb[3][6];                  // bounding box of chunk m in bb[m % 3]: min x, y, z, max x, y, z (cells)
+    int org[2][3];                 // origin of the box in stage s
+    int fit[2];                    // stage s holds the box of its chunk (else: gather from global memory)
+    int krange[2];                 // smallest first / largest last+1 interval index of the CTA's rays
+};
+
+template <int VW>
+__global__ void __launch_bounds__(kThreads, 3)
+gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtensorMap tmap) {
+    __shared__ StageCtl ctl;
+    float4* s_mu = reinterpret_cast<float4*>(s_box + 2 * kStageElems);
+    float2* s_src = reinterpret_cast<float2*>(s_mu + P.n_energy);
+    for (int e = threadIdx.x; e < P.n_energy; e += kThreads) {
+        s_mu[e] = P.mu_tab[e];
+        s_src[e] = P.src_tab[e];
+    }
+    if (threadIdx.x == 0) {
+        mbar_init(&ctl.bar[0], 1);
+        mbar_init(&ctl.bar[1], 1);
+        for (int m = 0; m < 3; ++m)
+            for (int a = 0; a < 3; ++a) { ctl.bb[m][a] = 0x7fffffff; ctl.bb[m][3 + a] = (int)0x80000000; }
+        ctl.krange[0] = 0x7fffffff;
+        ctl.krange[1] = (int)0x80000000;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    int i, j;
+    thread_pixel_map(i, j);
+    const int pl = blockIdx.z;
+    const int lane = threadIdx.x & 31;
+    const bool valid = i < P.g.nu && j < P.g.nv;
+
+    // ---- a1: ray setup (fp64) ------------------------------------------------
+    int j0, n;
+    Sampler S;
+    double gs[3], dg[3];
+    {
+        Ray r;
+        ray_setup(P.g, P.g.proj_begin + pl, min(i, P.g.nu - 1), min(j, P.g.nv - 1), r);
+        if (!valid) r.n = 0;
+        if (valid && P.ray_table) {
+            const size_t pix = ((size_t)pl * P.g.nv + j) * P.g.nu + i;
+            reinterpret_cast<int2*>(P.ray_table)[pix] = make_int2(r.j0, r.n);
+        }
+        index_line(P.g, r, gs, dg);
+        j0 = r.j0;
+        n = r.n;
+    }
+    S.dqx = __double2int_rn(dg[0] * 8388608.0);
+    S.dqy = __double2int_rn(dg[1] * 8388608.0);
+    S.dqz = __double2int_rn(dg[2] * 8388608.0);
+    S.sy = P.v.stride_y;
+    S.sz = P.v.stride_z;
+    S.vol0 = reinterpret_cast<const uint4*>(P.v.vox);
+    S.vol1 = reinterpret_cast<const uint4*>(P.v.vox1);
+    S.fmask = P.frac_mask;
+    S.fone = P.one_bits;
+    const unsigned un = (unsigned)n;
+
+    // interval range of the whole CTA: all its rays walk the same chunks of kStageK indices
+    {
+        const int wmin = __reduce_min_sync(0xffffffffu, n > 0 ? j0 : 0x7fffffff);
+        const int wmax = __reduce_max_sync(0xffffffffu, n > 0 ? j0 + n : (int)0x80000000);
+        if (lane == 0 && wmin < wmax) {
+            atomicMin(&ctl.krange[0], wmin);
+            atomicMax(&ctl.krange[1], wmax);
+        }
+    }
+    __syncthreads();
+    const int kmin = ctl.krange[0], kmax = ctl.krange[1];
+
+    float acc[VW];
+#pragma unroll
+    for (int m = 0; m < VW; ++m) acc[m] = 0.f;
+    RayAcc<VW> A;
+    A.cur = 0.f;
+    A.curm4 = 4u;
+
+    if (kmin < kmax) {
+        const int c_begin = kmin / kStageK;
+        const int nchunks = (kmax - 1) / kStageK - c_begin + 1;
+
+        // base position of chunk m, and this ray's share of the chunk's bounding box -> ctl.bb[m % 3]
+        auto prepare = [&](int m, ChunkBase& b) {
+            const int kc = (c_begin + m) * kStageK;
+            b = chunk_base(gs, dg, kc);
+            const int lo = max(j0 - kc, 0), hi = min(j0 + n - kc, kStageK);
+            int mn[3] = {0x7fffffff, 0x7fffffff, 0x7fffffff};
+            int mx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+            if (hi > lo) {                       // cells of the first and the last sample, exactly as the loop forms them
+                const int bc[3] = {b.cx, b.cy, b.cz}, bq[3] = {b.qx, b.qy, b.qz}, dq[3] = {S.dqx, S.dqy, S.dqz};
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const int c_lo = bc[a] + ((bq[a] + lo * dq[a]) >> kFracBits);
+                    const int c_hi = bc[a] + ((bq[a] + (hi - 1) * dq[a]) >> kFracBits);
+                    mn[a] = min(c_lo, c_hi);
+                    mx[a] = max(c_lo, c_hi);
+                }
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                mn[a] = __reduce_min_sync(0xffffffffu, mn[a]);
+                mx[a] = __reduce_max_sync(0xffffffffu, mx[a]);
+            }
+            if (lane == 0 && mn[0] <= mx[0]) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    atomicMin(&ctl.bb[m % 3][a], mn[a]);
+                    atomicMax(&ctl.bb[m % 3][3 + a], mx[a]);
+                }
+            }
+        };
+        // thread 0: request the box of chunk m into stage m & 1 if it fits
+        auto issue = [&](int m) {
+            const int* bb = ctl.bb[m % 3];
+            const int st = m & 1;
+            const bool fit = bb[0] <= bb[3] && bb[3] - bb[0] + 1 <= kBX && bb[4] - bb[1] + 1 <= kBY &&
+                             bb[5] - bb[2] + 2 <= kBZ;
+            ctl.fit[st] = fit;
+            ctl.org[st][0] = bb[0];
+            ctl.org[st][1] = bb[1];
+            ctl.org[st][2] = bb[2];
+            if (fit) {
+                mbar_arrive_expect_tx(&ctl.bar[st], kBoxBytes);
+                tma_load_box(s_box + st * kStageElems, &tmap, 4 * bb[0], bb[1], bb[2], &ctl.bar[st]);
+            }
+        };
+
+        ChunkBase b_cur, b_next;
+        prepare(0, b_cur);
+        b_next = b_cur;
+        __syncthreads();
+        if (threadIdx.x == 0) issue(0);
+        unsigned phase[2] = {0u, 0u};
+
+        for (int m = 0; m < nchunks; ++m) {
+            const int st = m & 1;
+            if (threadIdx.x == 0) {              // the slot chunk m + 2 will use: consumed two iterations ago
+                for (int a = 0; a < 3; ++a) { ctl.bb[(m + 2) % 3][a] = 0x7fffffff; ctl.bb[(m + 2) % 3][3 + a] = (int)0x80000000; }
+            }
+            if (m + 1 < nchunks) prepare(m + 1, b_next);
+            __syncthreads();                     // box of m + 1 known; everyone is done with stage st ^ 1
+            if (threadIdx.x == 0 && m + 1 < nchunks) issue(m + 1);
+
+            const int kc = (c_begin + m) * kStageK;
+            const unsigned rel = (unsigned)(kc - j0);
+            const bool mine = rel < un && rel + (unsigned)kStageK <= un;     // this lane owns the whole chunk
+            const bool all_mine = __all_sync(0xffffffffu, mine);
+#pragma unroll
+            for (int k = 0; k < VW; ++k) A.part[k] = 0.f;
+
+            if (ctl.fit[st]) {
+                mbar_wait(&ctl.bar[st], phase[st]);
+                phase[st] ^= 1u;
+                const int idx0 = st * kStageElems + ((b_cur.cz - ctl.org[st][2]) * kBY + (b_cur.cy - ctl.org[st][1])) * kBX +
+                                 (b_cur.cx - ctl.org[st][0]);
+                if (all_mine) run_chunk_staged<VW, false>(S, b_cur.qx, b_cur.qy, b_cur.qz, idx0, kStageK, rel, un, A);
+                else run_chunk_staged<VW, true>(S, b_cur.qx, b_cur.qy, b_cur.qz, idx0, kStageK, rel, un, A);
+            } else {
+                if (all_mine) run_chunk<VW, false>(S, b_cur, kStageK, rel, un, A);
+                else run_chunk<VW, true>(S, b_cur, kStageK, rel, un, A);
+            }
+            add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur);
+            A.cur = 0.f;
+#pragma unroll
+            for (int k = 0; k < VW; ++k) acc[k] += A.part[k];
+            b_cur = b_next;
+        }
+    }
+
+    if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, P.g.step, pl, i, j);
+}
+
+template <int VW>
+static cudaError_t launch_staged_t(const ProjectParams& p, const CUtensorMap& map, cudaStream_t s) {
+    dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
+    const size_t smem = 2 * (size_t)kStageElems * 16 + (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(gdrr_project_staged_kernel<VW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             2 * kStageElems * 16 + 512 * 24 /* GDRR_MAX_ENERGIES bins */);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    gdrr_project_staged_kernel<VW><<<grid, kThreads, smem, s>>>(p, map);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_project_staged(const ProjectParams& p, int vw, const void* tensor_map, cudaStream_t s) {
+    const CUtensorMap& map = *reinterpret_cast<const CUtensorMap*>(tensor_map);
+    if (vw == 1) return launch_staged_t<1>(p, map, s);
+    if (vw == 2) return launch_staged_t<2>(p, map, s);
+    return launch_staged_t<4>(p, map, s);
+}
+
+}  // namespace gdrr
