@@ -210,7 +210,9 @@ def run_b200(args):
     launch_proj = per_gpu if args.launch_proj <= 0 else min(args.launch_proj, per_gpu)
 
     pr = g.Projector(w, device=local_rank, layout=args.layout,
-                     method=g.GDRR_METHOD_SIDDON if args.method == "siddon" else g.GDRR_METHOD_TRILINEAR)
+                     method=g.GDRR_METHOD_SIDDON if args.method == "siddon" else g.GDRR_METHOD_TRILINEAR,
+                     sampler={"auto": g.GDRR_SAMPLER_AUTO, "gather": g.GDRR_SAMPLER_GATHER,
+                              "staged": g.GDRR_SAMPLER_STAGED}[args.sampler])
     signal = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32, device=dev)
     stream = torch.cuda.current_stream()
     if args.method == "siddon":                            # units = voxel segments of positive length
@@ -318,7 +320,8 @@ def run_b200(args):
     hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
     kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
-             "gdrr_project_packed_kernel" if args.layout == 2 else "gdrr_project_kernel")
+             "gdrr_project_kernel" if args.layout != 2 else
+             "gdrr_project_packed_kernel" if args.sampler == "gather" else "gdrr_project_staged_kernel")
     roofline = {"kernel": kname, "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
                 "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
                 "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),
@@ -341,7 +344,7 @@ def run_b200(args):
                "sample": f"{sample} ({n} samples)",
                "max_rel_err_of_b200_signal_on_sample": float(np.max(np.abs(got - ref) / ref))}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "method": args.method, "n_gpus": world, "steps": args.steps,
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "method": args.method, "sampler": args.sampler, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
@@ -365,6 +368,8 @@ def main():
     ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
     ap.add_argument("--method", default="trilinear", choices=sorted(METHODS),
                     help="line integral: the paper's default tri-linear midpoint rule, or its Siddon option")
+    ap.add_argument("--sampler", default="auto", choices=["auto", "gather", "staged"],
+                    help="packed-quad sampling kernel: quads staged through shared memory by TMA (auto), or gathered through L1")
     ap.add_argument("--angle-deg", type=float, default=None,
                     help="profiling aid: all projections at this one gantry angle instead of an evenly spaced scan")
     ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")

@@ -191,9 +191,17 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
         const int nchunks = (kmax - 1) / kStageK - c_begin + 1;
 
         // base position of chunk m, and this ray's share of the chunk's bounding box -> ctl.bb[m % 3]
-        auto prepare = [&](int m, ChunkBase& b) {
+        // (every 4th chunk the base is re-formed in fp64; in between it is the previous base advanced by
+        // kStageK steps in the loop's own fixed-point arithmetic: drift <= 64 * 2^-24 voxel)
+        auto prepare = [&](int m, int slot, ChunkBase& b) {
             const int kc = (c_begin + m) * kStageK;
-            b = chunk_base(gs, dg, kc);
+            if ((m & 3) == 0) {
+                b = chunk_base(gs, dg, kc);
+            } else {
+                const int qx = b.qx + kStageK * S.dqx, qy = b.qy + kStageK * S.dqy, qz = b.qz + kStageK * S.dqz;
+                b.cx += qx >> kFracBits; b.cy += qy >> kFracBits; b.cz += qz >> kFracBits;
+                b.qx = qx & ((1 << kFracBits) - 1); b.qy = qy & ((1 << kFracBits) - 1); b.qz = qz & ((1 << kFracBits) - 1);
+            }
             const int lo = max(j0 - kc, 0), hi = min(j0 + n - kc, kStageK);
             int mn[3] = {0x7fffffff, 0x7fffffff, 0x7fffffff};
             int mx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
@@ -215,14 +223,14 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             if (lane == 0 && mn[0] <= mx[0]) {
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
-                    atomicMin(&ctl.bb[m % 3][a], mn[a]);
-                    atomicMax(&ctl.bb[m % 3][3 + a], mx[a]);
+                    atomicMin(&ctl.bb[slot][a], mn[a]);
+                    atomicMax(&ctl.bb[slot][3 + a], mx[a]);
                 }
             }
         };
         // thread 0: request the box of chunk m into stage m & 1 if it fits
-        auto issue = [&](int m) {
-            const int* bb = ctl.bb[m % 3];
+        auto issue = [&](int m, int slot) {
+            const int* bb = ctl.bb[slot];
             const int st = m & 1;
             const bool fit = bb[0] <= bb[3] && bb[3] - bb[0] + 1 <= kBX && bb[4] - bb[1] + 1 <= kBY &&
                              bb[5] - bb[2] + 2 <= kBZ;
@@ -237,20 +245,26 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
         };
 
         ChunkBase b_cur, b_next;
-        prepare(0, b_cur);
+        prepare(0, 0, b_cur);
         b_next = b_cur;
         __syncthreads();
-        if (threadIdx.x == 0) issue(0);
+        if (threadIdx.x == 0) issue(0, 0);
         unsigned phase[2] = {0u, 0u};
+        int slot1 = 1, slot2 = 2;                // bounding-box slots of chunks m + 1 and m + 2 (m % 3 rotation)
 
         for (int m = 0; m < nchunks; ++m) {
             const int st = m & 1;
             if (threadIdx.x == 0) {              // the slot chunk m + 2 will use: consumed two iterations ago
-                for (int a = 0; a < 3; ++a) { ctl.bb[(m + 2) % 3][a] = 0x7fffffff; ctl.bb[(m + 2) % 3][3 + a] = (int)0x80000000; }
+                for (int a = 0; a < 3; ++a) { ctl.bb[slot2][a] = 0x7fffffff; ctl.bb[slot2][3 + a] = (int)0x80000000; }
             }
-            if (m + 1 < nchunks) prepare(m + 1, b_next);
+            if (m + 1 < nchunks) prepare(m + 1, slot1, b_next);
             __syncthreads();                     // box of m + 1 known; everyone is done with stage st ^ 1
-            if (threadIdx.x == 0 && m + 1 < nchunks) issue(m + 1);
+            if (threadIdx.x == 0 && m + 1 < nchunks) issue(m + 1, slot1);
+            {
+                const int s0 = 3 - slot1 - slot2;    // rotate (slot of m, slot1, slot2) -> (slot1, slot2, slot of m)
+                slot1 = slot2;
+                slot2 = s0;
+            }
 
             const int kc = (c_begin + m) * kStageK;
             const unsigned rel = (unsigned)(kc - j0);
@@ -285,13 +299,10 @@ template <int VW>
 static cudaError_t launch_staged_t(const ProjectParams& p, const CUtensorMap& map, cudaStream_t s) {
     dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
     const size_t smem = 2 * (size_t)kStageElems * 16 + (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(gdrr_project_staged_kernel<VW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             2 * kStageElems * 16 + 512 * 24 /* GDRR_MAX_ENERGIES bins */);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // per device and cheap: set at every launch (the boxes alone exceed the 48 KB default)
+    cudaError_t e = cudaFuncSetAttribute(gdrr_project_staged_kernel<VW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         2 * kStageElems * 16 + 512 * 24 /* GDRR_MAX_ENERGIES bins */);
+    if (e != cudaSuccess) return e;
     gdrr_project_staged_kernel<VW><<<grid, kThreads, smem, s>>>(p, map);
     return cudaGetLastError();
 }
