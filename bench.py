@@ -321,7 +321,9 @@ def run_b200(args):
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
     kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
              "gdrr_project_kernel" if args.layout != 2 else
-             "gdrr_project_packed_kernel" if args.sampler == "gather" else "gdrr_project_staged_kernel")
+             "gdrr_project_packed_kernel" if args.sampler == "gather" else
+             "gdrr_project_staged_kernel" if args.sampler == "staged" else
+             "gdrr_project_staged_kernel (auto: gdrr_project_packed_kernel when a CTA's beam cannot fit the staged box)")
     roofline = {"kernel": kname, "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
                 "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
                 "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),

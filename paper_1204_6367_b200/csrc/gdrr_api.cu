@@ -261,8 +261,17 @@ bool make_tensor_map(gdrr_volume* v) {
 
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
     if (vol->ctx->method == GDRR_METHOD_SIDDON) return launch_project_siddon(P, vol->vw, vol->layout, s);
-    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && vol->ctx->sampler != GDRR_SAMPLER_GATHER)
-        return launch_project_staged(P, vol->vw, &vol->tmap, s);
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && vol->ctx->sampler != GDRR_SAMPLER_GATHER) {
+        // AUTO: staging pays when the beam of a 16 x 16-pixel CTA over 16 steps fits the 14 x 14 x 11-quad box
+        // (a chunk that does not fit is gathered anyway, after paying for its bounding box)
+        const gdrr_context* c = vol->ctx;
+        const double mag = c->sad / c->sdd;
+        const double fu = 16.0 * c->du * mag / std::fmin(vol->d[0], vol->d[1]);
+        const double fv = 16.0 * c->dv * mag / vol->d[2];
+        const double adv = 16.0 * P.g.step / std::fmin(vol->d[0], vol->d[1]);
+        const bool fits = fu <= 10.0 && fv <= 8.5 && adv <= 9.0;
+        if (fits || c->sampler == GDRR_SAMPLER_STAGED) return launch_project_staged(P, vol->vw, &vol->tmap, s);
+    }
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);
 }
