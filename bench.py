@@ -24,6 +24,7 @@ if ROOT not in sys.path:
 METRIC = "trilinear_samples_per_s"
 UNIT = "samples/s"
 METHODS = {"trilinear": ("trilinear_samples_per_s", "samples/s"),
+           "texture": ("texture_filtered_samples_per_s", "samples/s"),   # the paper's own design, reported separately
            "siddon": ("siddon_voxel_segments_per_s", "segments/s")}   # the paper's optional line integral
 SM_COUNT = 148
 L1_BYTES_PER_CLK = 128          # per SM, DESIGN.md "Roofline"
@@ -210,7 +211,8 @@ def run_b200(args):
     launch_proj = per_gpu if args.launch_proj <= 0 else min(args.launch_proj, per_gpu)
 
     pr = g.Projector(w, device=local_rank, layout=args.layout,
-                     method=g.GDRR_METHOD_SIDDON if args.method == "siddon" else g.GDRR_METHOD_TRILINEAR,
+                     method={"siddon": g.GDRR_METHOD_SIDDON, "texture": g.GDRR_METHOD_TEXTURE,
+                             "trilinear": g.GDRR_METHOD_TRILINEAR}[args.method],
                      sampler={"auto": g.GDRR_SAMPLER_AUTO, "gather": g.GDRR_SAMPLER_GATHER,
                               "staged": g.GDRR_SAMPLER_STAGED}[args.sampler])
     signal = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32, device=dev)
@@ -320,6 +322,7 @@ def run_b200(args):
     hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
     kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
+             "gdrr_project_texture_kernel" if args.method == "texture" else
              "gdrr_project_kernel" if args.layout != 2 else
              "gdrr_project_packed_kernel" if args.sampler == "gather" else
              "gdrr_project_staged_kernel" if args.sampler == "staged" else
@@ -384,7 +387,9 @@ def main():
     args = ap.parse_args()
     global METRIC, UNIT
     METRIC, UNIT = METHODS[args.method]
-    time_oracle.method = args.method
+    time_oracle.method = "siddon" if args.method == "siddon" else "trilinear"
+    if args.method == "texture":
+        args.layout = 1                                     # the texture is built from the LINEAR layout
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -85,8 +85,11 @@ enum {
 /* How the line integrals of Eq. (1) are evaluated. */
 enum {
     GDRR_METHOD_TRILINEAR = 0,   /* the paper's default: fixed-step midpoint rule on the tri-linear field */
-    GDRR_METHOD_SIDDON = 1       /* the paper's option: Siddon's exact radiological path through
+    GDRR_METHOD_SIDDON = 1,      /* the paper's option: Siddon's exact radiological path through
                                     homogeneous voxels, LI_m = sum_voxels rho [mat = m] |ray /\ voxel| */
+    GDRR_METHOD_TEXTURE = 2      /* the paper's own GPU design: the midpoint rule with the
+                                    hardware's 9-bit-weight texture filtering; optional, reported separately,
+                                    cannot meet the 1e-4 bar; needs gdrr_volume_attach_texture */
 };
 
 /* Which kernel samples a PACKED_QUAD volume with the tri-linear method.  Both give the same
@@ -212,6 +215,15 @@ GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int pr
  * layout (on PACKED_QUAD it reads the first word of each quad).
  * Errors: INVALID_ARG (unknown method). */
 GDRR_API int gdrr_set_method(gdrr_context* ctx, int method);
+
+/* Optional texture variant.  Copies a GDRR_LAYOUT_LINEAR volume into a 3-D CUDA
+ * array (one fp32 channel per material, 1, 2 or 4 channels) and makes a texture object with linear
+ * filtering, clamp addressing and unnormalised coordinates.  THE ONE PLACE THE LIBRARY ALLOCATES
+ * VOLUME-SIZED DEVICE MEMORY ITSELF (a CUDA array cannot be caller memory); it is freed by
+ * gdrr_destroy_volume.  Synchronises cuda_stream.  gdrr_project then uses the texture when the
+ * context's method is GDRR_METHOD_TEXTURE.
+ * Errors: INVALID_ARG (volume not LINEAR), CUDA. */
+GDRR_API int gdrr_volume_attach_texture(gdrr_context* ctx, gdrr_volume* vol, void* cuda_stream);
 
 /* Selects the sampling kernel for PACKED_QUAD volumes (default GDRR_SAMPLER_AUTO).
  * Errors: INVALID_ARG (unknown value). */

@@ -32,6 +32,7 @@ GDRR_SAMPLER_GATHER = 1
 GDRR_SAMPLER_STAGED = 2
 GDRR_METHOD_TRILINEAR = 0
 GDRR_METHOD_SIDDON = 1
+GDRR_METHOD_TEXTURE = 2
 GDRR_MAX_MATERIALS = 4
 GDRR_MAX_ENERGIES = 512
 
@@ -40,7 +41,7 @@ EXPORTS = (
     "gdrr_volume_workspace_bytes", "gdrr_create_volume", "gdrr_create_volume_host",
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
-    "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler",
+    "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture",
 )
 
 
@@ -73,6 +74,7 @@ def _load():
         "gdrr_ray_setup": (i, [vp, vp, i, i, vp, vp, vp]),
         "gdrr_set_method": (i, [vp, i]),
         "gdrr_set_sampler": (i, [vp, i]),
+        "gdrr_volume_attach_texture": (i, [vp, vp, vp]),
         "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
         "gdrr_kernel_launches": (ctypes.c_ulonglong, [vp]),
         "gdrr_version": (ctypes.c_char_p, []),
@@ -265,6 +267,10 @@ def gdrr_set_method(ctx, method):
     _check(_lib.gdrr_set_method(ctx, int(method)), ctx)
 
 
+def gdrr_volume_attach_texture(ctx, vol, stream=None):
+    _check(_lib.gdrr_volume_attach_texture(ctx, vol, _stream(stream)), ctx)
+
+
 def gdrr_set_sampler(ctx, sampler):
     _check(_lib.gdrr_set_sampler(ctx, int(sampler)), ctx)
 
@@ -295,6 +301,7 @@ class Projector:
         self.ctx = gdrr_create_context(device)
         self.vol = None
         self.layout = layout
+        self.method = method
         gdrr_set_method(self.ctx, method)
         gdrr_set_sampler(self.ctx, sampler)
         gdrr_set_geometry(self.ctx, w.sad, w.sdd, w.theta, w.nu, w.nv, w.du, w.dv, w.u_off, w.v_off,
@@ -321,6 +328,8 @@ class Projector:
         with self.torch.cuda.device(self.device):
             self.vol = gdrr_create_volume(self.ctx, self.rho_stage, self.mat_stage, w.dims, w.spacing,
                                           w.centre, w.n_materials, self.layout, self.workspace)
+            if self.method == GDRR_METHOD_TEXTURE:
+                gdrr_volume_attach_texture(self.ctx, self.vol)
 
     def ingest_host(self, rho_host, mat_host):
         """Step a0 from host buffers (H2D copy inside the library call)."""

@@ -53,6 +53,8 @@ struct gdrr_volume {
     int n_mat, vw, layout;
     int sy, sz;                 // PACKED_QUAD: element strides
     bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
+    cudaArray_t tex_array = nullptr;     // optional texture variant (gdrr_volume_attach_texture)
+    cudaTextureObject_t tex = 0;
     alignas(64) CUtensorMap tmap;
 };
 
@@ -201,6 +203,8 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     if (!ctx->has_spec) return fail(ctx, GDRR_ERR_NOT_READY, "gdrr_set_spectrum has not been called");
     if (ctx->n_mat != vol->n_mat)
         return fail(ctx, GDRR_ERR_NOT_READY, "spectrum has %d materials, volume has %d", ctx->n_mat, vol->n_mat);
+    if (ctx->method == GDRR_METHOD_TEXTURE && !vol->tex)
+        return fail(ctx, GDRR_ERR_NOT_READY, "GDRR_METHOD_TEXTURE needs gdrr_volume_attach_texture on this volume");
     P.v.vox = vol->vox;
     P.v.nvox[0] = vol->nx; P.v.nvox[1] = vol->ny; P.v.nvox[2] = vol->nz;
     P.seg_table = nullptr;
@@ -261,6 +265,7 @@ bool make_tensor_map(gdrr_volume* v) {
 
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
     if (vol->ctx->method == GDRR_METHOD_SIDDON) return launch_project_siddon(P, vol->vw, vol->layout, s);
+    if (vol->ctx->method == GDRR_METHOD_TEXTURE) return launch_project_texture(P, vol->vw, (unsigned long long)vol->tex, s);
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && vol->ctx->sampler != GDRR_SAMPLER_GATHER) {
         // AUTO: staging pays when the beam of a 16 x 16-pixel CTA over 16 steps fits the 14 x 14 x 11-quad box
         // (a chunk that does not fit is gathered anyway, after paying for its bounding box)
@@ -415,6 +420,11 @@ int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host, const uint
 }
 
 int gdrr_destroy_volume(gdrr_volume* vol) {
+    if (vol && (vol->tex || vol->tex_array)) {
+        DeviceGuard guard(vol->ctx->device);
+        if (vol->tex) cudaDestroyTextureObject(vol->tex);
+        if (vol->tex_array) cudaFreeArray(vol->tex_array);
+    }
     delete vol;
     return GDRR_OK;
 }
@@ -601,9 +611,51 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
 
 int gdrr_set_method(gdrr_context* ctx, int method) {
     if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
-    if (method != GDRR_METHOD_TRILINEAR && method != GDRR_METHOD_SIDDON)
+    if (method != GDRR_METHOD_TRILINEAR && method != GDRR_METHOD_SIDDON && method != GDRR_METHOD_TEXTURE)
         return fail(ctx, GDRR_ERR_INVALID_ARG, "unknown method %d", method);
     ctx->method = method;
+    return GDRR_OK;
+}
+
+int gdrr_volume_attach_texture(gdrr_context* ctx, gdrr_volume* vol, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!vol || vol->ctx != ctx) return fail(ctx, GDRR_ERR_INVALID_ARG, "volume is NULL or belongs to another context");
+    if (vol->layout != GDRR_LAYOUT_LINEAR)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "the texture variant is built from a GDRR_LAYOUT_LINEAR volume");
+    if (vol->tex) return GDRR_OK;
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int vw = vol->vw;
+    const cudaChannelFormatDesc desc = cudaCreateChannelDesc(32, vw > 1 ? 32 : 0, vw > 2 ? 32 : 0, vw > 2 ? 32 : 0,
+                                                             cudaChannelFormatKindFloat);
+    const cudaExtent ext = make_cudaExtent((size_t)vol->px, (size_t)vol->py, (size_t)vol->pz);
+    cudaError_t e = cudaMalloc3DArray(&vol->tex_array, &desc, ext);
+    if (e != cudaSuccess) { vol->tex_array = nullptr; return cuda_fail(ctx, e, "cudaMalloc3DArray"); }
+    cudaMemcpy3DParms cp = {};
+    cp.srcPtr = make_cudaPitchedPtr(vol->vox, (size_t)vol->px * vw * sizeof(float), (size_t)vol->px, (size_t)vol->py);
+    cp.dstArray = vol->tex_array;
+    cp.extent = ext;
+    cp.kind = cudaMemcpyDeviceToDevice;
+    e = cudaMemcpy3DAsync(&cp, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) {
+        cudaResourceDesc res = {};
+        res.resType = cudaResourceTypeArray;
+        res.res.array.array = vol->tex_array;
+        cudaTextureDesc td = {};
+        td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+        td.filterMode = cudaFilterModeLinear;
+        td.readMode = cudaReadModeElementType;
+        td.normalizedCoords = 0;
+        e = cudaCreateTextureObject(&vol->tex, &res, &td, nullptr);
+    }
+    if (e != cudaSuccess) {
+        cudaFreeArray(vol->tex_array);
+        vol->tex_array = nullptr;
+        vol->tex = 0;
+        return cuda_fail(ctx, e, "building the texture");
+    }
     return GDRR_OK;
 }
 

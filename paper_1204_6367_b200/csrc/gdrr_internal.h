@@ -70,6 +70,7 @@ cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cud
 cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
 // tensor_map: a CUtensorMap over the packed-quad volume (3-D: words along x, rows, slabs; box 4*14 x 14 x 11)
 cudaError_t launch_project_staged(const ProjectParams& p, int vw, const void* tensor_map, cudaStream_t s);
+cudaError_t launch_project_texture(const ProjectParams& p, int vw, unsigned long long tex_object, cudaStream_t s);
 cudaError_t launch_project_siddon(const ProjectParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
