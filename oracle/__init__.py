@@ -40,7 +40,8 @@ def _load():
         build()
         _lib = ctypes.CDLL(_LIB)
         for name in ("gdrr_oracle_ray", "gdrr_oracle_trilinear", "gdrr_oracle_ray_samples",
-                     "gdrr_oracle_project", "gdrr_oracle_project_siddon", "gdrr_oracle_project_literal"):
+                     "gdrr_oracle_project", "gdrr_oracle_project_siddon", "gdrr_oracle_project_literal",
+                     "gdrr_oracle_denoise"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -187,6 +188,20 @@ def project_literal(w, pixels, step=None, n_threads=0):
     if rc:
         raise ValueError("gdrr_oracle_project_literal: invalid arguments")
     return dict(signal=signal, tau=tau)
+
+
+def denoise(s_hat, beta, n_iter, omega=0.8, floor=1e-12, s0=None):
+    """Relaxed Jacobi sweeps of the paper's Eq. (5) on one image [nv][nu]; fp64."""
+    lib = _load()
+    s_hat = np.ascontiguousarray(s_hat, dtype=np.float64)
+    nv, nu = s_hat.shape
+    s0a = None if s0 is None else np.ascontiguousarray(s0, dtype=np.float64)
+    out, work = np.zeros_like(s_hat), np.zeros_like(s_hat)
+    rc = lib.gdrr_oracle_denoise(_dp(s_hat), _dp(s0a), ctypes.c_int(nu), ctypes.c_int(nv), ctypes.c_double(beta),
+                                 ctypes.c_double(omega), ctypes.c_int(n_iter), ctypes.c_double(floor), _dp(out), _dp(work))
+    if rc:
+        raise ValueError("gdrr_oracle_denoise: invalid arguments")
+    return out
 
 
 def n_threads_available() -> int:

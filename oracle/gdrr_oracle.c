@@ -566,4 +566,50 @@ int gdrr_oracle_project_literal(const float *rho, const uint8_t *mat,
     return 0;
 }
 
+/*
+ * Scatter denoising, PAPER.md:199-218 (section 2.5).  The noisy scatter image S_hat is modelled as
+ * Poisson with a smooth mean S minimising  E[S] = Int (S - S_hat log S) + beta/2 Int |grad S|^2
+ * (Eq. (2)); with the 5-point Laplacian the optimality condition is Eq. (4)
+ * and the paper iterates Eq. (5):
+ *
+ *   S(k+1)(i,j) = (1 - w) S(k)(i,j) + w/4 [ Sum S(k)(i,j) - 1/beta (1 - S_hat(i,j) / S(k)(i,j)) ],
+ *   Sum S(i,j) = S(i+1,j) + S(i,j+1) + S(i-1,j) + S(i,j-1),   w = 0.8,   S(0) = S_hat.
+ *
+ * Every value on the right is of iteration k (a relaxed Jacobi sweep), exactly as printed.
+ * Readings where the paper is silent: [Q28] neighbours outside the detector are replaced by the
+ * nearest pixel inside (replicate = zero normal derivative, the natural boundary condition of
+ * the |grad S|^2 penalty); [Q29] S is kept >= floor > 0 (S(0) = max(S_hat, floor), each iterate
+ * clamped) so that S_hat / S is defined where the Monte Carlo image has empty pixels; [Q30] a
+ * fixed number of sweeps n_iter (the paper gives no stopping rule).
+ *   s_hat  in  [nv][nu];  s0 in [nv][nu] or NULL (= s_hat);  s_out out [nv][nu];  work [nv][nu] scratch
+ * Returns 0, or -1 on invalid arguments.
+ */
+int gdrr_oracle_denoise(const double *s_hat, const double *s0, int nu, int nv, double beta, double omega,
+                        int n_iter, double floor_value, double *s_out, double *work)
+{
+    if (!s_hat || !s_out || !work || nu <= 0 || nv <= 0 || !(beta > 0.0) || n_iter < 0 || !(floor_value > 0.0))
+        return -1;
+    double *cur = s_out, *nxt = work;
+    for (int q = 0; q < nu * nv; ++q) {
+        double v = s0 ? s0[q] : s_hat[q];
+        cur[q] = v > floor_value ? v : floor_value;
+    }
+    for (int k = 0; k < n_iter; ++k) {
+        for (int j = 0; j < nv; ++j) {
+            for (int i = 0; i < nu; ++i) {
+                int ip = i + 1 < nu ? i + 1 : nu - 1, im = i > 0 ? i - 1 : 0;       /* [Q28] */
+                int jp = j + 1 < nv ? j + 1 : nv - 1, jm = j > 0 ? j - 1 : 0;
+                double s = cur[j * nu + i];
+                double sum = cur[j * nu + ip] + cur[jp * nu + i] + cur[j * nu + im] + cur[jm * nu + i];
+                double v = (1.0 - omega) * s + (omega / 4.0) * (sum - (1.0 / beta) * (1.0 - s_hat[j * nu + i] / s));
+                nxt[j * nu + i] = v > floor_value ? v : floor_value;                    /* [Q29] */
+            }
+        }
+        double *t = cur; cur = nxt; nxt = t;
+    }
+    if (cur != s_out)
+        for (int q = 0; q < nu * nv; ++q) s_out[q] = cur[q];
+    return 0;
+}
+
 int gdrr_oracle_max_materials(void) { return GDRR_ORACLE_MAX_MATERIALS; }
