@@ -362,6 +362,82 @@ def run_b200(args):
     pr.close()
 
 
+def run_denoise(args):
+    """--method denoise: the scatter denoiser of PAPER.md:199-218 on a scan of synthetic
+    Poisson images; a step = n_iter sweeps of Eq. (5) on every image."""
+    import torch
+    import paper_1204_6367_b200 as g
+    from workloads import make_workload
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU path")
+    w = make_workload(args.workload)
+    n_img = w.n_proj if args.projections <= 0 else args.projections
+    n_iter, beta = 100, 0.2
+    peaks = measured_peaks()
+    gen = torch.Generator(device="cuda").manual_seed(12046367)
+    jj = torch.arange(w.nv, device="cuda")[:, None].float()
+    ii = torch.arange(w.nu, device="cuda")[None, :].float()
+    truth = 40.0 * (0.4 + torch.exp(-((ii - 0.4 * w.nu) ** 2 / (0.1 * w.nu ** 2) + (jj - 0.6 * w.nv) ** 2 / (0.2 * w.nv ** 2))))
+    s_hat = torch.poisson(truth.expand(n_img, -1, -1).contiguous(), generator=gen) + 1.0
+    out, scratch = torch.empty_like(s_hat), torch.empty_like(s_hat)
+    ctx = g.gdrr_create_context(0)
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        g.gdrr_denoise_scatter(ctx, s_hat, out, scratch, beta, n_iter)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    l0 = g.gdrr_kernel_launches(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        g.gdrr_denoise_scatter(ctx, s_hat, out, scratch, beta, n_iter)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    launches = g.gdrr_kernel_launches(ctx) - l0
+    units = n_img * w.nu * w.nv * n_iter
+    value = units * args.steps / (ms * 1e-3)
+    # e2e: host images in, denoised images out
+    hin, hout = s_hat.cpu().pin_memory(), torch.empty(s_hat.shape).pin_memory()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        s_hat.copy_(hin, non_blocking=True)
+        g.gdrr_denoise_scatter(ctx, s_hat, out, scratch, beta, n_iter)
+        hout.copy_(out, non_blocking=True)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    import oracle
+    img = s_hat[0].cpu().numpy()
+    t0 = time.perf_counter()
+    ref = oracle.denoise(img, beta=beta, n_iter=n_iter)
+    dt = time.perf_counter() - t0
+    err = float(np.max(np.abs(out[0].cpu().numpy() - ref) / ref))
+    bytes_per_unit = 12.0 / 4                                  # S and S_hat in, S out, once per 4 fused sweeps
+    achieved = bytes_per_unit * units * args.steps / (ms * 1e-3) / 1e9
+    line = {"metric": "denoise_pixel_sweeps_per_s", "value": value, "unit": "pixel-sweeps/s", "method": "denoise",
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic (seeded Poisson images of a smooth scatter-like field)",
+            "config": {"workload": f"{args.workload} detector, scatter denoiser (PAPER.md:199-218)", "detector": [w.nu, w.nv],
+                       "images": n_img, "sweeps": n_iter, "beta": beta, "omega": 0.8,
+                       "l2": "three image stacks exceed L2 (no flush needed)" if 3 * s_hat.numel() * 4 > 126e6 else "fits L2"},
+            "images_per_s": n_img * args.steps / (ms * 1e-3),
+            "paper_context": "paper: 0.041 s per projection for denoising + noise calibration on a GTX 580 (PAPER.md:366)",
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": units * args.steps / (e2e_ms * 1e-3), "unit": "pixel-sweeps/s",
+                    "h2d_bytes_per_step": int(hin.numel() * 4), "d2h_bytes_per_step": int(hout.numel() * 4)},
+            "roofline": {"kernel": "gdrr_denoise_kernel", "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": None,
+                         "algorithmic": "12 B per pixel per launch of 4 fused sweeps = 3 B per pixel-sweep",
+                         "peak_source": peaks["source"]},
+            "cpu_baseline": {"value": img.size * n_iter / dt, "unit": "pixel-sweeps/s", "cores": 1, "kind": "oracle",
+                             "sample": "one image", "max_rel_err_of_b200_on_sample": err}}
+    print(json.dumps(line), flush=True)
+    g.gdrr_destroy_context(ctx)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -371,7 +447,7 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--projections", type=int, default=0, help="projections per GPU (0 = the workload's)")
     ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
-    ap.add_argument("--method", default="trilinear", choices=sorted(METHODS),
+    ap.add_argument("--method", default="trilinear", choices=sorted(METHODS) + ["denoise"],
                     help="line integral: the paper's default tri-linear midpoint rule, or its Siddon option")
     ap.add_argument("--sampler", default="auto", choices=["auto", "gather", "staged"],
                     help="packed-quad sampling kernel: quads staged through shared memory by TMA (auto), or gathered through L1")
@@ -386,6 +462,10 @@ def main():
                     help="dram bytes per launch from the committed ncu capture (profiles/)")
     args = ap.parse_args()
     global METRIC, UNIT
+    if args.method == "denoise":
+        if args.impl == "reference" or args.gpus != 1:
+            raise SystemExit("--method denoise is a single-GPU measurement of the b200 arm")
+        return run_denoise(args)
     METRIC, UNIT = METHODS[args.method]
     time_oracle.method = "siddon" if args.method == "siddon" else "trilinear"
     if args.method == "texture":

@@ -242,6 +242,22 @@ GDRR_API int gdrr_ray_setup(gdrr_context* ctx, const gdrr_volume* vol, int proj_
                    int32_t* ray_table_dev, unsigned long long* n_samples_dev,
                    void* cuda_stream);
 
+/* ---- scatter denoising: PAPER.md:199-218 (section 2.5) ---------------------- */
+
+/* n_iter relaxed Jacobi sweeps of the paper's Eq. (5) on n_images detector images:
+ *   S(k+1) = (1 - omega) S(k) + omega/4 [ Sum S(k) - 1/beta (1 - S_hat / S(k)) ],  S(0) = S_hat,
+ * Sum = the four edge neighbours, all of sweep k.  Outside the detector the nearest pixel inside is
+ * used (replicated edge); S is kept >= floor_value > 0 (S(0) = max(S_hat, floor), every iterate
+ * clamped) so that empty Monte Carlo pixels are defined.  The paper uses omega = 0.8.
+ *   s_hat_dev    in  [n_images][nv][nu] fp32 (the noisy scatter image)
+ *   s_dev        out [n_images][nv][nu] fp32
+ *   scratch_dev  work, same size as s_dev
+ * Asynchronous on cuda_stream.  Errors: INVALID_ARG (NULLs, sizes, beta <= 0, floor <= 0, n_iter < 0,
+ * omega outside (0, 2)), CUDA. */
+GDRR_API int gdrr_denoise_scatter(gdrr_context* ctx, const float* s_hat_dev, float* s_dev, float* scratch_dev,
+                         int nu, int nv, int n_images, double beta, double omega, int n_iter,
+                         double floor_value, void* cuda_stream);
+
 /* Number of kernels this library has launched on ctx since creation (for the
  * harness's gpu_launches count). */
 GDRR_API unsigned long long gdrr_kernel_launches(const gdrr_context* ctx);

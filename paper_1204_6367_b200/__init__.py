@@ -41,7 +41,7 @@ EXPORTS = (
     "gdrr_volume_workspace_bytes", "gdrr_create_volume", "gdrr_create_volume_host",
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
-    "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture",
+    "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture", "gdrr_denoise_scatter",
 )
 
 
@@ -75,6 +75,7 @@ def _load():
         "gdrr_set_method": (i, [vp, i]),
         "gdrr_set_sampler": (i, [vp, i]),
         "gdrr_volume_attach_texture": (i, [vp, vp, vp]),
+        "gdrr_denoise_scatter": (i, [vp, vp, vp, vp, i, i, i, d, d, i, d, vp]),
         "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
         "gdrr_kernel_launches": (ctypes.c_ulonglong, [vp]),
         "gdrr_version": (ctypes.c_char_p, []),
@@ -269,6 +270,16 @@ def gdrr_set_method(ctx, method):
 
 def gdrr_volume_attach_texture(ctx, vol, stream=None):
     _check(_lib.gdrr_volume_attach_texture(ctx, vol, _stream(stream)), ctx)
+
+
+def gdrr_denoise_scatter(ctx, s_hat_dev, s_dev, scratch_dev, beta, n_iter, omega=0.8, floor_value=1e-12, stream=None):
+    """s_hat_dev, s_dev, scratch_dev: float32 CUDA tensors [n_images][nv][nu] (or [nv][nu])."""
+    shape = tuple(s_hat_dev.shape)
+    n_images, nv, nu = (1,) + shape if len(shape) == 2 else shape
+    n = n_images * nv * nu
+    _check(_lib.gdrr_denoise_scatter(ctx, _dev(s_hat_dev, "float32", n, "s_hat_dev"), _dev(s_dev, "float32", n, "s_dev"),
+                                     _dev(scratch_dev, "float32", n, "scratch_dev"), nu, nv, n_images, float(beta),
+                                     float(omega), int(n_iter), float(floor_value), _stream(stream)), ctx)
 
 
 def gdrr_set_sampler(ctx, sampler):

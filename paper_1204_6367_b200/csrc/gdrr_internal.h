@@ -75,4 +75,7 @@ cudaError_t launch_project_siddon(const ProjectParams& p, int vw, int layout, cu
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 
+cudaError_t launch_denoise(const float* s_hat, float* s_dev, float* scratch, int nu, int nv, int n_images,
+                           double beta, double omega, int n_iter, double floor_value, cudaStream_t st, int* launches);
+
 }  // namespace gdrr
