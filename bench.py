@@ -334,6 +334,11 @@ def run_b200(args):
                 "algorithmic": f"{per_unit} voxel value(s) x {corner_bytes} B = {per_unit * corner_bytes} B per "
                                f"{'segment' if args.method == 'siddon' else 'sample'} through L1",
                 "samples_per_clk_per_sm": n_samples / (kernel_ms * 1e-3) / (SM_COUNT * peaks["sm_max_mhz"] * 1e6),
+                "ncu_identified_bound": {
+                    "gdrr_project_staged_kernel": "instruction issue: 78.9% of issue slots, L1 data pipe 57% (profiles/r01_staged_kernel_ncu.md)",
+                    "gdrr_project_packed_kernel": "L1 data-pipe wavefronts: 72% over a scan, 85-89% on one angle (profiles/r01_packed_kernel_ncu.md)",
+                    "gdrr_project_siddon_kernel": "load latency: issue 45%, L1 19% (profiles/r01_siddon_kernel_ncu.md)",
+                }.get(kname.split(" ")[0], "not profiled"),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
                         "algorithmic": "device-layout volume once per projection + 4 B per pixel"}}
