@@ -275,7 +275,8 @@ cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaS
         const double fv = 16.0 * c->dv * mag / vol->d[2];
         const double adv = 16.0 * P.g.step / std::fmin(vol->d[0], vol->d[1]);
         const bool fits = fu <= 10.0 && fv <= 8.5 && adv <= 9.0;
-        if (fits || c->sampler == GDRR_SAMPLER_STAGED) return launch_project_staged(P, vol->vw, &vol->tmap, s);
+        // (the staged kernel walks chunks of 16 steps: P.chunk < 16 means 16 steps would overflow the 9.23 fixed point)
+        if (P.chunk >= 16 && (fits || c->sampler == GDRR_SAMPLER_STAGED)) return launch_project_staged(P, vol->vw, &vol->tmap, s);
     }
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);

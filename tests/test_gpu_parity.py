@@ -90,6 +90,13 @@ def test_both_packed_samplers_against_the_oracle(gdrr, workloads_cache, sampler)
                       phis=np.radians([15.0, 100.0, 222.0]), step=0.5, mu_hat=rng.uniform(0.01, 0.03, size=(3, 1)))
     with gdrr.Projector(w, sampler=sampler) as pr:
         compare_full(pr, w, oracle.project(w), f"ragged sampler {sampler}")
+    # long steps: 2.5 voxels per step (no chunk fits the staged box) and 10 voxels per step (16 steps would
+    # overflow the in-chunk fixed point: the library must fall back to the gather kernel's short chunks)
+    for step in (2.5, 10.0):
+        ws = tiny_workload(rho, mat, n_materials=3, spacing=(1.0, 1.0, 1.3), nu=45, nv=39, du=0.8, dv=0.8,
+                           phis=np.radians([15.0, 222.0]), step=step, mu_hat=rng.uniform(0.01, 0.03, size=(3, 1)))
+        with gdrr.Projector(ws, sampler=sampler) as pr:
+            compare_full(pr, ws, oracle.project(ws), f"step {step} sampler {sampler}")
 
 
 def test_staged_and_gather_samplers_agree(gdrr, workloads_cache):
