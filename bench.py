@@ -313,6 +313,12 @@ def run_b200(args):
         return
 
     # ---- roofline of the dominant kernel (gdrr_project_kernel) ----------------------
+    kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
+             "gdrr_project_texture_kernel" if args.method == "texture" else
+             "gdrr_project_kernel" if args.layout != 2 else
+             "gdrr_project_packed_kernel" if args.sampler == "gather" else
+             "gdrr_project_staged_kernel" if args.sampler == "staged" else
+             "gdrr_project_staged_kernel (auto: gdrr_project_packed_kernel when a CTA's beam cannot fit the staged box)")
     corner_bytes = 4 if args.layout == 2 else 4 * vw        # packed word, or one float per material
     per_unit = 1 if args.method == "siddon" else 8          # one voxel per segment, 8 corners per sample
     l1_bytes = per_unit * corner_bytes * n_samples
@@ -320,13 +326,14 @@ def run_b200(args):
     l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
     hbm_bytes = per_gpu * (vol_bytes + w.nu * w.nv * 4)
     hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
+    # dram__bytes_read + dram__bytes_write per launch, from the committed `ncu --set full` captures (8 projections of
+    # C3 per launch; per-projection figure x the projections of one launch here); other workloads: not captured
+    NCU_DRAM_PER_PROJECTION = {("C3", "gdrr_project_staged_kernel"): (3.392058e9 + 11.2704e6) / 8,      # profiles/r01_staged_kernel_ncu.md
+                               ("C3", "gdrr_project_packed_kernel"): (3.194201e9 + 10.405888e6) / 8,    # profiles/r01_packed_kernel_ncu.md
+                               ("C3", "gdrr_project_siddon_kernel"): (3.158578e9 + 12.190208e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
-    kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
-             "gdrr_project_texture_kernel" if args.method == "texture" else
-             "gdrr_project_kernel" if args.layout != 2 else
-             "gdrr_project_packed_kernel" if args.sampler == "gather" else
-             "gdrr_project_staged_kernel" if args.sampler == "staged" else
-             "gdrr_project_staged_kernel (auto: gdrr_project_packed_kernel when a CTA's beam cannot fit the staged box)")
+    if ncu_traffic is None and (args.workload, kname.split(" ")[0]) in NCU_DRAM_PER_PROJECTION:
+        ncu_traffic = NCU_DRAM_PER_PROJECTION[(args.workload, kname.split(" ")[0])] * launch_proj
     roofline = {"kernel": kname, "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
                 "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
                 "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),

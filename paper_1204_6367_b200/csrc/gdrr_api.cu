@@ -52,6 +52,7 @@ struct gdrr_volume {
     double d[3], c[3];
     int n_mat, vw, layout;
     int sy, sz;                 // PACKED_QUAD: element strides
+    void* compact = nullptr;    // PACKED_QUAD: bricked one-word-per-voxel copy (Siddon walk)
     bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
     cudaArray_t tex_array = nullptr;     // optional texture variant (gdrr_volume_attach_texture)
     cudaTextureObject_t tex = 0;
@@ -121,6 +122,11 @@ size_t packed_elements(int nx, int ny, int nz) {
     stored_dims(nx, ny, nz, GDRR_LAYOUT_PACKED_QUAD, px, py, pz);
     packed_strides(px, py, sy, sz);
     return (size_t)sz * pz;
+}
+
+// bytes of the 4 x 4 x 2-bricked one-word-per-voxel copy kept behind the quads (Siddon walk)
+size_t compact_bytes(int nx, int ny, int nz) {
+    return (size_t)((nx + 3) / 4) * ((ny + 3) / 4) * ((nz + 1) / 2) * 128;
 }
 
 size_t element_bytes(int n_mat, int layout) {
@@ -208,6 +214,9 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     P.v.vox = vol->vox;
     P.v.nvox[0] = vol->nx; P.v.nvox[1] = vol->ny; P.v.nvox[2] = vol->nz;
     P.seg_table = nullptr;
+    P.v.compact = vol->compact;
+    P.v.cstride_y = 32 * ((vol->nx + 3) / 4);
+    P.v.cstride_z = 32 * ((vol->nx + 3) / 4) * ((vol->ny + 3) / 4);
     if (vol->layout == GDRR_LAYOUT_BRICK) {
         P.v.stride_y = 8 * (vol->px / 2);
         P.v.stride_z = 8 * (vol->px / 2) * (vol->py / 2);
@@ -334,7 +343,7 @@ int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int lay
     int px, py, pz;
     stored_dims(nx, ny, nz, layout, px, py, pz);
     *bytes = (size_t)px * py * pz * element_bytes(n_materials, layout);
-    if (layout == GDRR_LAYOUT_PACKED_QUAD) *bytes = 16 * packed_elements(nx, ny, nz);
+    if (layout == GDRR_LAYOUT_PACKED_QUAD) *bytes = ((16 * packed_elements(nx, ny, nz) + 255) & ~(size_t)255) + compact_bytes(nx, ny, nz);
     return GDRR_OK;
 }
 
@@ -371,7 +380,11 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     stored_dims(nx, ny, nz, layout, ip.px, ip.py, ip.pz);
     ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev;
     ip.sy = ip.sz = 0;
-    if (layout == GDRR_LAYOUT_PACKED_QUAD) packed_strides(ip.px, ip.py, ip.sy, ip.sz);
+    ip.compact = nullptr; ip.cbx = (nx + 3) / 4; ip.cby = (ny + 3) / 4;
+    if (layout == GDRR_LAYOUT_PACKED_QUAD) {
+        packed_strides(ip.px, ip.py, ip.sy, ip.sz);
+        ip.compact = (char*)workspace_dev + ((16 * (size_t)ip.sz * ip.pz + 255) & ~(size_t)255);
+    }
     const int vw = vector_width(n_materials);
     e = launch_ingest(ip, vw, layout, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel launch");
@@ -389,7 +402,7 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     v->d[0] = dx_mm; v->d[1] = dy_mm; v->d[2] = dz_mm;
     for (int a = 0; a < 3; ++a) v->c[a] = centre_mm ? centre_mm[a] : 0.0;
     v->n_mat = n_materials; v->vw = vw; v->layout = layout;
-    v->sy = ip.sy; v->sz = ip.sz;
+    v->sy = ip.sy; v->sz = ip.sz; v->compact = ip.compact;
     v->has_tmap = layout == GDRR_LAYOUT_PACKED_QUAD && make_tensor_map(v);
     *out = v;
     return GDRR_OK;

@@ -34,6 +34,8 @@ struct VolumeParams {
     const void* vox1;               // PACKED_QUAD: vox + one slab (its own parameter: one IMAD.WIDE per load)
     int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: elements per row (= 3 mod 8)
     int nvox[3];                    // nx, ny, nz (Siddon traversal)
+    const void* compact;            // PACKED_QUAD: one tagged word per voxel in 4 x 4 x 2 bricks of 128 B (Siddon walk)
+    int cstride_y, cstride_z;       //   words per row of bricks, per slab of bricks
     int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab (= 4 mod 8)
 };
 
@@ -60,6 +62,8 @@ struct IngestParams {
     int nx, ny, nz;
     int px, py, pz;                 // stored dims (voxels for BRICK / LINEAR, quads for PACKED_QUAD)
     int sy, sz;                     // PACKED_QUAD: element strides (VolumeParams)
+    void* compact;                  // PACKED_QUAD: the 4 x 4 x 2-bricked one-word-per-voxel copy
+    int cbx, cby;                   //   bricks per row, rows of bricks per slab
     int n_mat;
     int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
 };

@@ -13,7 +13,8 @@
 // Segments of zero or negative length (ties at lattice edges, rounding) contribute nothing.
 //
 // Works on every device layout: the exact ones hold VW floats per voxel (one per material),
-// PACKED_QUAD is read through the first word of each quad (rho with its material tag).
+// a PACKED_QUAD volume carries a second, compact copy for this walk: the same tagged word per
+// voxel in 4 x 4 x 2 bricks of 128 B (4 B per voxel instead of 16, ~4 voxels of any walk per line).
 // fp32 accumulation is chunked like the tri-linear sampler's (32 segments per partial sum).
 #include "project_common.cuh"
 
@@ -42,11 +43,16 @@ __device__ __forceinline__ void add_routed_s(float (&part)[VW], int m, float v) 
     for (int k = 0; k < VW; ++k) part[k] += (m == k) ? v : 0.f;
 }
 
-// element offset of padded voxel index i along one axis (project_fused.cu has the same map)
+// Element offset contributed by voxel index i along one axis.  LAYOUT 0: padded 2x2x2 bricks of the exact
+// BRICK layout (project_fused.cu has the same map); 1: padded linear; 2: the packed volume's compact copy,
+// unpadded bricks of 4 (x) x 4 (y) x 2 (z) words (volume_layout.cu).
 template <int LAYOUT, int AXIS>
 __device__ __forceinline__ int siddon_axis_offset(int i, int stride) {
-    if (LAYOUT == 0) return (i >> 1) * stride + ((i & 1) << AXIS);
-    return i * stride;
+    if (LAYOUT == 0) return ((i + 1) >> 1) * stride + (((i + 1) & 1) << AXIS);
+    if (LAYOUT == 1) return (i + 1) * stride;
+    if (AXIS == 0) return (i >> 2) * 32 + (i & 3);
+    if (AXIS == 1) return (i >> 2) * stride + ((i & 3) << 2);
+    return (i >> 1) * stride + ((i & 1) << 4);
 }
 
 // len x voxel value into the per-material sums.  Exact layouts: one FMA per material.  Packed word:
@@ -75,11 +81,10 @@ template <int VW> struct SiddonVoxel<VW, 2> { using T = unsigned; };
 template <int VW, int LAYOUT>
 __device__ __forceinline__ typename SiddonVoxel<VW, LAYOUT>::T load_voxel(const void* vox, int off) {
     using T = typename SiddonVoxel<VW, LAYOUT>::T;
-    if (LAYOUT == 2) return __ldg(reinterpret_cast<const T*>(vox) + 4 * (size_t)off);     // first word of the quad
     return __ldg(reinterpret_cast<const T*>(vox) + off);
 }
 
-// LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed quad (first word of a quad)
+// LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed volume's compact bricked words
 // COUNT: also count the segments of positive length (gdrr_siddon_segments)
 template <int VW, int LAYOUT, bool COUNT>
 __global__ void __launch_bounds__(kThreads)
@@ -135,9 +140,10 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
         // steps out of the lattice; the sliver it may drop is < 5e-4 mm of the last voxel.
         const float t_stop = t_end * (1.f - 16.f * 5.96e-8f);
         constexpr int sx = (LAYOUT == 0) ? 8 : 1;
-        const int sy = P.v.stride_y, sz = P.v.stride_z;
-        int off = siddon_axis_offset<LAYOUT, 0>(idx[0] + 1, sx) + siddon_axis_offset<LAYOUT, 1>(idx[1] + 1, sy) +
-                  siddon_axis_offset<LAYOUT, 2>(idx[2] + 1, sz);
+        const int sy = LAYOUT == 2 ? P.v.cstride_y : P.v.stride_y, sz = LAYOUT == 2 ? P.v.cstride_z : P.v.stride_z;
+        const void* vox = LAYOUT == 2 ? P.v.compact : P.v.vox;
+        int off = siddon_axis_offset<LAYOUT, 0>(idx[0], sx) + siddon_axis_offset<LAYOUT, 1>(idx[1], sy) +
+                  siddon_axis_offset<LAYOUT, 2>(idx[2], sz);
         // linear element orders: stepping one voxel along an axis adds a constant to the element offset
         const int dox = stp[0] * sx, doy = stp[1] * sy, doz = stp[2] * sz;
         float kx = 0.f, ky = 0.f, kz = 0.f;              // planes crossed so far per axis (exact in fp32)
@@ -147,7 +153,7 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
         float cur = 0.f;
 
         // the voxel of segment s + 1 is requested before segment s is accumulated
-        VT v = load_voxel<VW, LAYOUT>(P.v.vox, off);
+        VT v = load_voxel<VW, LAYOUT>(vox, off);
         bool more = true;
         while (more) {
             float part[VW];
@@ -161,12 +167,12 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
                 // cross the plane that was met (x before y before z at ties), branch-free
                 const bool bx = tx <= ty && tx <= tz;
                 const bool by = !bx && ty <= tz;
-                if (LAYOUT == 0) {
+                if (LAYOUT != 1) {
                     idx[0] += bx ? stp[0] : 0;
                     idx[1] += by ? stp[1] : 0;
                     idx[2] += (bx || by) ? 0 : stp[2];
-                    off = siddon_axis_offset<0, 0>(idx[0] + 1, sx) + siddon_axis_offset<0, 1>(idx[1] + 1, sy) +
-                          siddon_axis_offset<0, 2>(idx[2] + 1, sz);
+                    off = siddon_axis_offset<LAYOUT, 0>(idx[0], sx) + siddon_axis_offset<LAYOUT, 1>(idx[1], sy) +
+                          siddon_axis_offset<LAYOUT, 2>(idx[2], sz);
                 } else {
                     off += bx ? dox : (by ? doy : doz);
                 }
@@ -174,7 +180,7 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
                 else if (by) { ky += 1.f; ty = fmaf(ky, dt[1], t0[1]); }
                 else { kz += 1.f; tz = fmaf(kz, dt[2], t0[2]); }
                 const VT cv = v;
-                if (more) v = load_voxel<VW, LAYOUT>(P.v.vox, off);
+                if (more) v = load_voxel<VW, LAYOUT>(vox, off);
                 if (len > 0.f) {
                     if (COUNT) ++n_seg;
                     accumulate_voxel<VW, LAYOUT>(cv, len, part, cur, curm);

@@ -107,6 +107,31 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
     reinterpret_cast<uint4*>(P.vox)[o] = out;
 }
 
+// PACKED_QUAD, second copy for the Siddon walk (project_siddon.cu): the same tagged word per voxel
+// (no pad, no purity flag), stored once, in bricks of 4 (x) x 4 (y) x 2 (z) voxels = one 128-byte line,
+// bricks x fastest.  A walk then finds ~4 consecutive voxels in a line whatever its direction, and a
+// 4-byte warp-wide load touches a few sectors instead of one per lane.  One thread per stored word.
+__global__ void __launch_bounds__(256)
+gdrr_ingest_compact_kernel(const IngestParams P) {
+    const size_t total = (size_t)P.cbx * P.cby * ((P.nz + 1) / 2) * 32;
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= total) return;
+    const int e = (int)(o & 31);
+    size_t b = o >> 5;
+    const int bx = (int)(b % P.cbx);
+    b /= P.cbx;
+    const int by = (int)(b % P.cby);
+    const int bz = (int)(b / P.cby);
+    const int ix = 4 * bx + (e & 3), iy = 4 * by + ((e >> 2) & 3), iz = 2 * bz + (e >> 4);
+    unsigned bits = 0u;
+    if (ix < P.nx && iy < P.ny && iz < P.nz) {
+        const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
+        bits = __float_as_uint(P.rho[src]);
+        if (P.n_mat > 1) bits = ((bits + 4u) & ~7u) | (P.mat[src] & 3u);
+    }
+    reinterpret_cast<unsigned*>(P.compact)[o] = bits;
+}
+
 template <int VW, int LAYOUT>
 static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
     const size_t total = (size_t)p.px * p.py * p.pz;
@@ -119,6 +144,10 @@ cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_
     if (layout == 2) {
         const size_t total = (size_t)p.sz * p.pz;
         gdrr_ingest_packed_kernel<<<(unsigned int)((total + 255) / 256), 256, 0, s>>>(p);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess || !p.compact) return e;
+        const size_t words = (size_t)p.cbx * p.cby * ((p.nz + 1) / 2) * 32;
+        gdrr_ingest_compact_kernel<<<(unsigned int)((words + 255) / 256), 256, 0, s>>>(p);
         return cudaGetLastError();
     }
     if (layout == 0) {
