@@ -330,7 +330,7 @@ def run_b200(args):
     # C3 per launch; per-projection figure x the projections of one launch here); other workloads: not captured
     NCU_DRAM_PER_PROJECTION = {("C3", "gdrr_project_staged_kernel"): (3.392058e9 + 11.2704e6) / 8,      # profiles/r01_staged_kernel_ncu.md
                                ("C3", "gdrr_project_packed_kernel"): (3.194201e9 + 10.405888e6) / 8,    # profiles/r01_packed_kernel_ncu.md
-                               ("C3", "gdrr_project_siddon_kernel"): (3.158578e9 + 12.190208e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
+                               ("C3", "gdrr_project_siddon_kernel"): (656.83712e6 + 10.174976e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
     if ncu_traffic is None and (args.workload, kname.split(" ")[0]) in NCU_DRAM_PER_PROJECTION:
         ncu_traffic = NCU_DRAM_PER_PROJECTION[(args.workload, kname.split(" ")[0])] * launch_proj
@@ -344,7 +344,7 @@ def run_b200(args):
                 "ncu_identified_bound": {
                     "gdrr_project_staged_kernel": "instruction issue: 78.9% of issue slots, L1 data pipe 57% (profiles/r01_staged_kernel_ncu.md)",
                     "gdrr_project_packed_kernel": "L1 data-pipe wavefronts: 72% over a scan, 85-89% on one angle (profiles/r01_packed_kernel_ncu.md)",
-                    "gdrr_project_siddon_kernel": "load latency: issue 45%, L1 19% (profiles/r01_siddon_kernel_ncu.md)",
+                    "gdrr_project_siddon_kernel": "instruction issue: 78% of issue slots, L1 13% (profiles/r01_siddon_kernel_ncu.md)",
                 }.get(kname.split(" ")[0], "not profiled"),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],

@@ -212,7 +212,7 @@ GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int pr
  * line integral of its material; the energy sum, the outputs and the ray table
  * (which stays the midpoint table of the geometry) are unchanged.  A ray that
  * lies IN a lattice plane belongs to either neighbour (a tie).  Works on every
- * layout (on PACKED_QUAD it reads the first word of each quad).
+ * layout (a PACKED_QUAD workspace carries a compact bricked copy for this walk).
  * Errors: INVALID_ARG (unknown method). */
 GDRR_API int gdrr_set_method(gdrr_context* ctx, int method);
 
