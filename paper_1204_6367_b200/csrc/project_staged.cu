@@ -215,17 +215,12 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
                     mx[a] = max(c_lo, c_hi);
                 }
             }
+            // every lane calls the atomics with its own values (neutral ones if it has no sample in the chunk):
+            // the compiler aggregates a warp-uniform shared atomic into one redux + one atomic by an elected lane
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                mn[a] = __reduce_min_sync(0xffffffffu, mn[a]);
-                mx[a] = __reduce_max_sync(0xffffffffu, mx[a]);
-            }
-            if (lane == 0 && mn[0] <= mx[0]) {
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    atomicMin(&ctl.bb[slot][a], mn[a]);
-                    atomicMax(&ctl.bb[slot][3 + a], mx[a]);
-                }
+                atomicMin(&ctl.bb[slot][a], mn[a]);
+                atomicMax(&ctl.bb[slot][3 + a], mx[a]);
             }
         };
         // thread 0: request the box of chunk m into stage m & 1 if it fits
