@@ -53,6 +53,7 @@ struct gdrr_volume {
     int n_mat, vw, layout;
     int sy, sz;                 // PACKED_QUAD: element strides
     void* compact = nullptr;    // PACKED_QUAD: bricked one-word-per-voxel copy (Siddon walk)
+    mutable bool compact_ready = false;   // ... made from the quads at the first Siddon use
     bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
     cudaArray_t tex_array = nullptr;     // optional texture variant (gdrr_volume_attach_texture)
     cudaTextureObject_t tex = 0;
@@ -272,8 +273,25 @@ bool make_tensor_map(gdrr_volume* v) {
     return r == CUDA_SUCCESS;
 }
 
+// Siddon on a packed volume walks the compact copy: make it (once, on the caller's stream) from the quads.
+cudaError_t ensure_compact(const gdrr_volume* vol, cudaStream_t s) {
+    if (vol->layout != GDRR_LAYOUT_PACKED_QUAD || vol->compact_ready) return cudaSuccess;
+    IngestParams ip = {};
+    ip.vox = vol->vox; ip.compact = vol->compact;
+    ip.nx = vol->nx; ip.ny = vol->ny; ip.nz = vol->nz;
+    ip.sy = vol->sy; ip.sz = vol->sz; ip.n_mat = vol->n_mat;
+    ip.cbx = (vol->nx + 3) / 4; ip.cby = (vol->ny + 3) / 4;
+    cudaError_t e = launch_compact_copy(ip, s);
+    if (e == cudaSuccess) { vol->compact_ready = true; vol->ctx->launches += 1; }
+    return e;
+}
+
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
-    if (vol->ctx->method == GDRR_METHOD_SIDDON) return launch_project_siddon(P, vol->vw, vol->layout, s);
+    if (vol->ctx->method == GDRR_METHOD_SIDDON) {
+        cudaError_t e = ensure_compact(vol, s);
+        if (e != cudaSuccess) return e;
+        return launch_project_siddon(P, vol->vw, vol->layout, s);
+    }
     if (vol->ctx->method == GDRR_METHOD_TEXTURE) return launch_project_texture(P, vol->vw, (unsigned long long)vol->tex, s);
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && vol->ctx->sampler != GDRR_SAMPLER_GATHER) {
         // AUTO: staging pays when the beam of a 16 x 16-pixel CTA over 16 steps fits the 14 x 14 x 11-quad box
@@ -710,7 +728,8 @@ int gdrr_siddon_segments(gdrr_context* ctx, const gdrr_volume* vol, int proj_beg
     P.signal = nullptr; P.li = nullptr; P.ray_table = nullptr; P.seg_table = n_segments_dev;
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
-    cudaError_t e = launch_project_siddon(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
+    cudaError_t e = ensure_compact(vol, (cudaStream_t)cuda_stream);
+    if (e == cudaSuccess) e = launch_project_siddon(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "Siddon kernel launch");
     ctx->launches += 1;
     return GDRR_OK;

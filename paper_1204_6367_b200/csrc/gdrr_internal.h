@@ -70,6 +70,8 @@ struct IngestParams {
 
 // Host-callable launchers (each returns the cudaGetLastError() of its launch).
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
+// PACKED_QUAD: fills p.compact (4 x 4 x 2-bricked words) from the quads in p.vox; needs nx..nz, sy, sz, cbx, cby, n_mat
+cudaError_t launch_compact_copy(const IngestParams& p, cudaStream_t s);
 cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
 // tensor_map: a CUtensorMap over the packed-quad volume (3-D: words along x, rows, slabs; box 4*14 x 14 x 11)

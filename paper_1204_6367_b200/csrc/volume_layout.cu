@@ -68,16 +68,16 @@ gdrr_ingest_kernel(const IngestParams P) {
 // freed bits: bits 0-1 the material index; bit 2, in the first word of an element
 // only, "the 8 corners of cell (ex, ey, ez) (this quad and the one above it in slab
 // ez + 1) all have this material".  Elements are stored linearly with strides sy, sz.
-// One thread per element slot; slots that are stride padding are zeroed.
+// One thread per element slot; slots that are stride padding are zeroed.  Grid: x over a row's sy slots
+// (+ the few pad slots between the last row and the slab pitch, taken by the blocks of the last row),
+// y = row, z = slab: no division in the index arithmetic.
 __global__ void __launch_bounds__(256)
 gdrr_ingest_packed_kernel(const IngestParams P) {
-    const size_t total = (size_t)P.sz * P.pz;
-    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= total) return;
-    const int ez = (int)(o / (size_t)P.sz);
-    const int rs = (int)(o - (size_t)ez * P.sz);
-    const int ey = rs / P.sy;
-    const int ex = rs - ey * P.sy;
+    const int ez = blockIdx.z, ey = blockIdx.y;
+    int ex = blockIdx.x * blockDim.x + threadIdx.x;
+    const int row_slots = (ey == P.py - 1) ? P.sz - ey * P.sy : P.sy;      // the last row also owns the slab's tail pad
+    if (ex >= row_slots) return;
+    const size_t o = (size_t)ez * P.sz + (size_t)ey * P.sy + ex;
     uint4 out = make_uint4(0u, 0u, 0u, 0u);
     if (ex < P.px && ey < P.py) {
         unsigned w[4];
@@ -107,27 +107,23 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
     reinterpret_cast<uint4*>(P.vox)[o] = out;
 }
 
-// PACKED_QUAD, second copy for the Siddon walk (project_siddon.cu): the same tagged word per voxel
-// (no pad, no purity flag), stored once, in bricks of 4 (x) x 4 (y) x 2 (z) voxels = one 128-byte line,
+// PACKED_QUAD, second copy for the Siddon walk (project_siddon.cu), made from the quads the first time the
+// Siddon method is used on a volume: the same tagged word per voxel (no pad, no purity flag), stored once, in bricks of 4 (x) x 4 (y) x 2 (z) voxels = one 128-byte line,
 // bricks x fastest.  A walk then finds ~4 consecutive voxels in a line whatever its direction, and a
 // 4-byte warp-wide load touches a few sectors instead of one per lane.  One thread per stored word.
 __global__ void __launch_bounds__(256)
 gdrr_ingest_compact_kernel(const IngestParams P) {
-    const size_t total = (size_t)P.cbx * P.cby * ((P.nz + 1) / 2) * 32;
-    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= total) return;
-    const int e = (int)(o & 31);
-    size_t b = o >> 5;
-    const int bx = (int)(b % P.cbx);
-    b /= P.cbx;
-    const int by = (int)(b % P.cby);
-    const int bz = (int)(b / P.cby);
+    // grid: x over the 32 cbx words of a row of bricks, y = row of bricks, z = slab of bricks
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 32 * P.cbx) return;
+    const int e = t & 31, bx = t >> 5, by = blockIdx.y, bz = blockIdx.z;
+    const size_t o = ((size_t)bz * P.cby + by) * P.cbx * 32 + t;
     const int ix = 4 * bx + (e & 3), iy = 4 * by + ((e >> 2) & 3), iz = 2 * bz + (e >> 4);
     unsigned bits = 0u;
     if (ix < P.nx && iy < P.ny && iz < P.nz) {
-        const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
-        bits = __float_as_uint(P.rho[src]);
-        if (P.n_mat > 1) bits = ((bits + 4u) & ~7u) | (P.mat[src] & 3u);
+        // voxel (ix, iy, iz) is the first word of quad (ix + 1, iy + 1, iz + 1); drop its purity flag
+        bits = reinterpret_cast<const unsigned*>(P.vox)[4 * ((size_t)(iz + 1) * P.sz + (size_t)(iy + 1) * P.sy + (ix + 1))];
+        if (P.n_mat > 1) bits &= ~4u;
     }
     reinterpret_cast<unsigned*>(P.compact)[o] = bits;
 }
@@ -140,14 +136,16 @@ static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
     return cudaGetLastError();
 }
 
+cudaError_t launch_compact_copy(const IngestParams& p, cudaStream_t s) {
+    gdrr_ingest_compact_kernel<<<dim3((32 * p.cbx + 255) / 256, p.cby, (p.nz + 1) / 2), 256, 0, s>>>(p);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s) {
     if (layout == 2) {
-        const size_t total = (size_t)p.sz * p.pz;
-        gdrr_ingest_packed_kernel<<<(unsigned int)((total + 255) / 256), 256, 0, s>>>(p);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess || !p.compact) return e;
-        const size_t words = (size_t)p.cbx * p.cby * ((p.nz + 1) / 2) * 32;
-        gdrr_ingest_compact_kernel<<<(unsigned int)((words + 255) / 256), 256, 0, s>>>(p);
+        // (py and pz, cby and nz / 2 stay far below the 65535 limit of grid.y / grid.z for any volume that fits int32 indexing)
+        const int row_max = p.sy + 8;                                   // a row, or the last row plus the slab's tail pad
+        gdrr_ingest_packed_kernel<<<dim3((row_max + 255) / 256, p.py, p.pz), 256, 0, s>>>(p);
         return cudaGetLastError();
     }
     if (layout == 0) {
