@@ -206,7 +206,7 @@ def _random_volume(rng, shape, n_mat):
 
 @pytest.mark.parametrize("layout", LAYOUTS)
 @pytest.mark.parametrize("case", ["ragged", "odd_aniso_offcentre", "theta_offset", "three_materials",
-                                  "long_step", "one_voxel", "thin_slab"])
+                                  "long_step", "one_voxel", "thin_slab", "long_thin"])
 def test_edge_cases(gdrr, case, layout):
     rng = np.random.default_rng(zlib.crc32(case.encode()))
     kw = dict(nu=37, nv=29, du=2.5, dv=2.5, step=0.5,
@@ -229,6 +229,9 @@ def test_edge_cases(gdrr, case, layout):
     elif case == "thin_slab":
         shape = (1, 24, 24)
         kw.update(step=0.25)
+    elif case == "long_thin":                         # 1500 voxels along x: cell indices beyond 1024, rays of 3000 samples
+        shape, spacing = (5, 6, 1500), (0.25, 0.5, 0.5)
+        kw.update(step=0.125, nu=40, nv=8, du=0.3, dv=0.3, phis=np.radians([0.0, 2.0, 90.0, 178.5]))
     rho, mat = _random_volume(rng, shape, n_mat)
     energies = np.array([30.0, 60.0, 90.0])
     mu_hat = rng.uniform(0.01, 0.05, size=(n_mat, 3))
