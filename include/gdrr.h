@@ -95,9 +95,11 @@ enum {
 /* Which kernel samples a PACKED_QUAD volume with the tri-linear method.  Both give the same
  * numbers to rounding order (the staged one sums in chunks of 16 samples, the gather one of 32). */
 enum {
-    GDRR_SAMPLER_AUTO = 0,     /* STAGED when the volume's tensor map could be made, else GATHER */
+    GDRR_SAMPLER_AUTO = 0,     /* STAGED when the volume's tensor map could be made and the beam of a 16 x 16-pixel
+                                  CTA over 16 steps can fit the 14 x 14 x 11-quad box; else GATHER */
     GDRR_SAMPLER_GATHER = 1,   /* quads gathered from global memory through L1 */
-    GDRR_SAMPLER_STAGED = 2    /* quads of a CTA's beam staged through shared memory by TMA */
+    GDRR_SAMPLER_STAGED = 2    /* quads of a CTA's beam staged through shared memory by TMA (a chunk whose beam
+                                  does not fit is gathered; GATHER is used if 16 steps exceed 120 voxels) */
 };
 
 #define GDRR_MAX_MATERIALS 4
@@ -115,7 +117,8 @@ GDRR_API const char* gdrr_last_error(const gdrr_context* ctx);
 
 /* ---- volume: step a0, PAPER.md:97 -------------------------------------- */
 
-/* Bytes of device workspace gdrr_create_volume needs for this shape. */
+/* Bytes of device workspace gdrr_create_volume needs for this shape (PACKED_QUAD: 16 B per quad with the
+ * skewed strides, rounded to 256, plus 4 B per voxel in 128-byte bricks for the Siddon walk's compact copy). */
 GDRR_API int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int layout,
                                 size_t* bytes);
 
