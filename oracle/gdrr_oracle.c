@@ -30,7 +30,9 @@
  * code), analytic sphere chord, additivity / linearity, literal-vs-factored
  * identity, z-mirror and 90-degree rotation equivariance, shadow of the box; for the
  * Siddon option: per-voxel box clipping (brute force), uniform-volume chord, axis-parallel
- * rows, nearest-neighbour fine-step limit.  No function here is "parity unpinned".
+ * rows, nearest-neighbour fine-step limit; for the scatter denoiser (tests/test_oracle_denoise_pins.py): a
+ * numpy sweep, the constant fixed point, the eigenmode amplification factor, Eq. (4) at convergence.
+ * No function here is "parity unpinned".
  *
  * Units: lengths mm, rho g/cm^3, mu_hat mm^-1 per g/cm^3, energies keV.
  * Build:  gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC ...

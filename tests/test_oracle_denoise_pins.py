@@ -69,3 +69,13 @@ def test_d5_floor_keeps_empty_pixels_defined():
     assert np.all(np.isfinite(out)) and out.min() >= 1e-3
     with pytest.raises(ValueError):
         oracle.denoise(s_hat, beta=0.0, n_iter=1)
+
+
+def test_denoise_golden_regression():
+    """tests/golden/oracle_denoise_regression.txt (written by tests/golden/make_golden.py from oracle/ only)."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_denoise_regression.txt")
+    want = np.array([[float(x) for x in l.split()] for l in open(path) if not l.startswith("#")])
+    rng = np.random.default_rng(12046367)
+    img = rng.poisson(30.0, size=(6, 8)).astype(np.float64) + 1.0
+    np.testing.assert_allclose(oracle.denoise(img, beta=0.25, n_iter=7), want, rtol=1e-13)

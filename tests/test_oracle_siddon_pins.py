@@ -132,3 +132,19 @@ def test_s6_material_routing_sums_to_the_unsegmented_volume(workloads_cache):
     tot = oracle.project(one, pixels=pix, method="siddon")
     np.testing.assert_allclose(seg["line_integrals"].sum(axis=1), tot["line_integrals"][:, 0], rtol=1e-12)
     assert (seg["line_integrals"][:, 1] > 0).any()               # bone is crossed somewhere
+
+
+def test_siddon_golden_regression(workloads_cache):
+    """tests/golden/oracle_siddon_regression.txt (written by tests/golden/make_golden.py, which calls only oracle/):
+    a guard against accidental changes of the oracle's arithmetic, not a pin."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_siddon_regression.txt")
+    rows = [l.split() for l in open(path) if not l.startswith("#")]
+    assert len(rows) == 10
+    for row in rows:
+        w = workloads_cache(row[0])
+        p, i, j, nseg = map(int, row[1:5])
+        out = oracle.project(w, pixels=np.array([[p, i, j]]), method="siddon")
+        assert int(out["n_segments"][0]) == nseg
+        assert out["signal"][0] == pytest.approx(float(row[5]), rel=1e-13)
+        assert np.allclose(out["line_integrals"][0], [float(x) for x in row[6:]], rtol=1e-13, atol=1e-13)
