@@ -90,6 +90,11 @@ def test_both_packed_samplers_against_the_oracle(gdrr, workloads_cache, sampler)
                       phis=np.radians([15.0, 100.0, 222.0]), step=0.5, mu_hat=rng.uniform(0.01, 0.03, size=(3, 1)))
     with gdrr.Projector(w, sampler=sampler) as pr:
         compare_full(pr, w, oracle.project(w), f"ragged sampler {sampler}")
+    # one material (untagged words, no purity vote) with a beam that fits the staged box
+    w1 = tiny_workload(rho, None, n_materials=1, spacing=(1.0, 1.0, 1.3), nu=45, nv=39, du=0.8, dv=0.8,
+                       phis=np.radians([15.0, 100.0, 222.0]), step=0.5)
+    with gdrr.Projector(w1, sampler=sampler) as pr:
+        compare_full(pr, w1, oracle.project(w1), f"one material sampler {sampler}")
     # long steps: 2.5 voxels per step (no chunk fits the staged box) and 10 voxels per step (16 steps would
     # overflow the in-chunk fixed point: the library must fall back to the gather kernel's short chunks)
     for step in (2.5, 10.0):
