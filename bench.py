@@ -346,6 +346,9 @@ def run_b200(args):
                     "gdrr_project_packed_kernel": "L1 data-pipe wavefronts: 72% over a scan, 85-89% on one angle (profiles/r01_packed_kernel_ncu.md)",
                     "gdrr_project_siddon_kernel": "instruction issue: 78% of issue slots, L1 13% (profiles/r01_siddon_kernel_ncu.md)",
                 }.get(kname.split(" ")[0], "not profiled"),
+                # busy fraction of that bound in the committed `ncu --set full` capture (8 projections of C3), not re-measured here
+                "ncu_bound_busy_frac": {"gdrr_project_staged_kernel": 0.783, "gdrr_project_packed_kernel": 0.715,
+                                        "gdrr_project_siddon_kernel": 0.781}.get(kname.split(" ")[0]),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
                         "algorithmic": "device-layout volume once per projection + 4 B per pixel"}}
