@@ -52,7 +52,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if res.returncode:
         raise RuntimeError("nvcc failed building libgdrr_b200.so")
     with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
-        f.write("$ " + " ".join(cmd) + "\n" + res.stderr)
+        # without the "Compile time" lines: they differ from build to build and the file is tracked
+        info = "\n".join(l for l in res.stderr.splitlines() if "Compile time" not in l)
+        f.write("$ " + " ".join(cmd) + "\n" + info + "\n")
     return LIB
 
 
