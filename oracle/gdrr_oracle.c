@@ -61,6 +61,9 @@ typedef struct {
     int nu, nv;
     double du, dv, u_off, v_off;
     double step;               /* dl */
+    /* general source paths (helical, C-arm; "with simple modifications"): per projection
+     * 12 doubles = source S, detector origin P, u_hat, v_hat; NULL = the circular gantry above */
+    const double *poses;
 } oracle_setup;
 
 typedef struct {
@@ -75,6 +78,15 @@ typedef struct {
 /* O1 + O2 + O3 + O4 of SURVEY.md section 8(c).  The order of the floating-point
  * operations below is part of the definition: (j0, n) is compared bit-exactly
  * with the CUDA path. */
+static void ray_from_points(const oracle_setup *g, const double D[3], oracle_ray *r);
+
+/* Pixel coordinates on the detector [Q4][Q5]. */
+static void pixel_uv(const oracle_setup *g, int i, int j, double *u, double *v)
+{
+    *u = ((double)i - 0.5 * (double)(g->nu - 1)) * g->du + g->u_off;
+    *v = ((double)j - 0.5 * (double)(g->nv - 1)) * g->dv + g->v_off;
+}
+
 static void ray_setup(const oracle_setup *g, double phi, int i, int j, oracle_ray *r)
 {
     /* O1: source on the circle of radius SAD; SO makes angle phi with +x,
@@ -90,12 +102,34 @@ static void ray_setup(const oracle_setup *g, double phi, int i, int j, oracle_ra
     r->S[2] = 0.0;
 
     /* O2: one ray through the pixel centre [Q4][Q5] */
-    double u = ((double)i - 0.5 * (double)(g->nu - 1)) * g->du + g->u_off;
-    double v = ((double)j - 0.5 * (double)(g->nv - 1)) * g->dv + g->v_off;
+    double u, v;
+    pixel_uv(g, i, j, &u, &v);
     double D[3];
     D[0] = Px + u * ux;
     D[1] = Py + u * uy;
     D[2] = v;
+    ray_from_points(g, D, r);
+}
+
+/* O1-G + O2 for a general pose [Q31]: the source and the detector frame are given per projection,
+ * pixel centre D = P + u u_hat + v v_hat, summed in that order.  With S, P, u_hat of the circular
+ * gantry and v_hat = +z this is ray_setup() bit for bit (tests/test_oracle_pose_pins.py). */
+static void ray_setup_pose(const oracle_setup *g, const double *pose, int i, int j, oracle_ray *r)
+{
+    const double *S = pose, *P = pose + 3, *uh = pose + 6, *vh = pose + 9;
+    double u, v;
+    pixel_uv(g, i, j, &u, &v);
+    double D[3];
+    for (int a = 0; a < 3; ++a) {
+        r->S[a] = S[a];
+        D[a] = (P[a] + u * uh[a]) + v * vh[a];
+    }
+    ray_from_points(g, D, r);
+}
+
+/* Tail of O2, O3, O4: the ray from r->S through the pixel centre D. */
+static void ray_from_points(const oracle_setup *g, const double D[3], oracle_ray *r)
+{
     double dx = D[0] - r->S[0], dy = D[1] - r->S[1], dz = D[2] - r->S[2];
     double L = sqrt((dx * dx + dy * dy) + dz * dz);
     r->L = L;
@@ -311,6 +345,7 @@ static int fill_setup(oracle_setup *g, const float *rho, const uint8_t *mat,
         step = 0.5 * m;
     }
     g->step = step;
+    g->poses = NULL;
     return 0;
 }
 
@@ -410,6 +445,7 @@ int gdrr_oracle_ray_samples(int nx, int ny, int nz, double dx, double dy, double
  * Returns 0, or -1 on invalid arguments.
  */
 static int project_impl(int method /* 0 tri-linear midpoint rule, 1 Siddon */, int32_t *n_segments,
+                        const double *poses /* [n_proj][12] or NULL = circular gantry */,
                         const float *rho, const uint8_t *mat,
                         int nx, int ny, int nz, double dx, double dy, double dz,
                         const double *centre, int n_materials,
@@ -426,9 +462,10 @@ static int project_impl(int method /* 0 tri-linear midpoint rule, 1 Siddon */, i
     oracle_setup g;
     if (fill_setup(&g, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd,
                    theta, nu, nv, du, dv, u_off, v_off, step)) return -1;
-    if (n_proj <= 0 || n_energy <= 0 || !phi || !phi_w || !resp || !mu_hat || !signal)
+    if (n_proj <= 0 || n_energy <= 0 || (!phi && !poses) || !phi_w || !resp || !mu_hat || !signal)
         return -1;
     if ((bt_mu == NULL) != (bt_thick == NULL)) return -1;
+    g.poses = poses;
     const int M = n_materials;
     const int64_t total = n_pix > 0 ? n_pix : (int64_t)n_proj * nv * nu;
     int bad = 0;
@@ -454,7 +491,8 @@ static int project_impl(int method /* 0 tri-linear midpoint rule, 1 Siddon */, i
         }
         oracle_ray r;
         double LI[GDRR_ORACLE_MAX_MATERIALS];
-        ray_setup(&g, phi[p], i, j, &r);
+        if (g.poses) ray_setup_pose(&g, g.poses + 12 * (size_t)p, i, j, &r);
+        else ray_setup(&g, phi[p], i, j, &r);
         if (method == 1) {
             int nseg = ray_siddon(&g, &r, LI);
             if (n_segments) n_segments[q] = nseg;
@@ -493,7 +531,7 @@ int gdrr_oracle_project(const float *rho, const uint8_t *mat,
                         double *signal, double *line_integrals, int32_t *ray_table,
                         int n_threads)
 {
-    return project_impl(0, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd, theta,
+    return project_impl(0, NULL, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd, theta,
                         nu, nv, du, dv, u_off, v_off, n_proj, phi, step, n_energy, phi_w, resp, mu_hat,
                         fluence, bt_mu, bt_thick, n_pix, pix, signal, line_integrals, ray_table, n_threads);
 }
@@ -513,10 +551,50 @@ int gdrr_oracle_project_siddon(const float *rho, const uint8_t *mat,
                         double *signal, double *line_integrals, int32_t *ray_table,
                         int32_t *n_segments, int n_threads)
 {
-    return project_impl(1, n_segments, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd,
+    return project_impl(1, n_segments, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd,
                         theta, nu, nv, du, dv, u_off, v_off, n_proj, phi, step, n_energy, phi_w, resp,
                         mu_hat, fluence, bt_mu, bt_thick, n_pix, pix, signal, line_integrals, ray_table,
                         n_threads);
+}
+
+/* The same projector (method 0 tri-linear, 1 Siddon) on a general source path [Q31]:
+ *   poses  [n_proj][12] = per projection source S, detector origin P, u_hat, v_hat (world, mm)
+ * The detector frame is used as given (u_hat, v_hat are expected to be unit and orthogonal). */
+int gdrr_oracle_project_poses(int method, const float *rho, const uint8_t *mat,
+                        int nx, int ny, int nz, double dx, double dy, double dz,
+                        const double *centre, int n_materials,
+                        int nu, int nv, double du, double dv, double u_off, double v_off,
+                        int n_proj, const double *poses, double step,
+                        int n_energy, const double *phi_w, const double *resp,
+                        const double *mu_hat, const float *fluence,
+                        const double *bt_mu, const double *bt_thick,
+                        int64_t n_pix, const int32_t *pix,
+                        double *signal, double *line_integrals, int32_t *ray_table,
+                        int32_t *n_segments, int n_threads)
+{
+    if (!poses || (method != 0 && method != 1)) return -1;
+    /* sad, sdd are not used on this path: any valid pair passes fill_setup */
+    return project_impl(method, method == 1 ? n_segments : NULL, poses, rho, mat, nx, ny, nz, dx, dy, dz,
+                        centre, n_materials, 1.0, 2.0, 0.0, nu, nv, du, dv, u_off, v_off, n_proj, NULL,
+                        step, n_energy, phi_w, resp, mu_hat, fluence, bt_mu, bt_thick, n_pix, pix, signal,
+                        line_integrals, ray_table, n_threads);
+}
+
+/* Geometry of one ray of a general pose; outputs as gdrr_oracle_ray. */
+int gdrr_oracle_ray_pose(int nx, int ny, int nz, double dx, double dy, double dz,
+                         const double *centre, int nu, int nv, double du, double dv,
+                         double u_off, double v_off, double step, const double *pose,
+                         int i, int j, double *out, int32_t *table)
+{
+    oracle_setup g;
+    if (!pose || fill_setup(&g, NULL, NULL, nx, ny, nz, dx, dy, dz, centre, 1, 1.0, 2.0, 0.0,
+                            nu, nv, du, dv, u_off, v_off, step)) return -1;
+    oracle_ray r;
+    ray_setup_pose(&g, pose, i, j, &r);
+    for (int a = 0; a < 3; ++a) { out[a] = r.S[a]; out[3 + a] = r.dir[a]; }
+    out[6] = r.L; out[7] = r.t_in; out[8] = r.t_out;
+    table[0] = r.j0; table[1] = r.n; table[2] = r.hit;
+    return 0;
 }
 
 /*

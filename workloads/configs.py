@@ -56,6 +56,9 @@ class Workload:
     bowtie_thickness: Optional[np.ndarray] = None  # float64 [nu] or None
     centre: tuple = (0.0, 0.0, 0.0)
     notes: dict = field(default_factory=dict)
+    # general source path (helical, C-arm): float64 [n_proj][12] = per projection source S, detector
+    # origin P, u_hat, v_hat (world, mm); None = the circular gantry (sad, sdd, theta, phis)
+    poses: Optional[np.ndarray] = None
 
     @property
     def dims(self):
@@ -64,7 +67,7 @@ class Workload:
 
     @property
     def n_proj(self):
-        return int(self.phis.shape[0])
+        return int(self.phis.shape[0] if self.poses is None else self.poses.shape[0])
 
     @property
     def n_energy(self):
@@ -75,6 +78,13 @@ class Workload:
         import copy
         w = copy.copy(self)
         w.phis = np.ascontiguousarray(np.asarray(phis, dtype=np.float64))
+        return w
+
+    def with_poses(self, poses):
+        """Same inputs on a general source path: poses [n_proj][12] (see workloads/trajectories.py)."""
+        import copy
+        w = copy.copy(self)
+        w.poses = np.ascontiguousarray(np.asarray(poses, dtype=np.float64)).reshape(-1, 12)
         return w
 
     def sha256(self):
