@@ -167,6 +167,21 @@ GDRR_API int gdrr_set_geometry(gdrr_context* ctx, double sad_mm, double sdd_mm, 
                       double u_offset_mm, double v_offset_mm,
                       int n_proj, const double* phi_rad, double step_mm);
 
+/* General source paths (other scanner geometries "with simple
+ * modifications"): instead of the circle, every projection p gives its own pose
+ *   poses [n_proj][12] = source S[3], detector origin P[3], u_hat[3], v_hat[3]   (host, copied; world, mm)
+ * and pixel (i, j)'s centre is D = (P + u u_hat) + v v_hat with (u, v) as above; the ray, its clipping,
+ * the midpoints and everything after are unchanged (reading Q31).  u_hat and v_hat are used
+ * as given (expected: unit and orthogonal).  A helix is the circle's pose with S_z and P_z advanced per
+ * projection; a C-arm orbit is the circle's poses rotated.  gdrr_set_geometry is this call with
+ * S = -SAD (cos phi, sin phi, 0), P = (SDD-SAD)(cos psi, sin psi, 0), u_hat = (-sin psi, cos psi, 0),
+ * v_hat = +z, psi = phi + theta, and gives bit-identical results.  The bowtie thickness table stays
+ * indexed by the pixel column i.
+ * Errors: INVALID_ARG (non-finite values, u_hat x v_hat = 0, source in the detector plane, sizes). */
+GDRR_API int gdrr_set_geometry_poses(gdrr_context* ctx, int nu, int nv, double du_mm, double dv_mm,
+                            double u_offset_mm, double v_offset_mm,
+                            int n_proj, const double* poses, double step_mm);
+
 /* ---- source and detector: PAPER.md:111, 117-121, 147-149 ---------------- */
 
 /*   phi_weight  [n_energy] per-channel spectrum weights, used as given

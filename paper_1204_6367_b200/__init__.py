@@ -42,6 +42,7 @@ EXPORTS = (
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
     "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture", "gdrr_denoise_scatter",
+    "gdrr_set_geometry_poses",
 )
 
 
@@ -68,6 +69,7 @@ def _load():
         "gdrr_create_volume_host": (i, [vp, vp, vp, i, i, i, d, d, d, vp, i, i, vp, vp, vp, sz, vp, pp]),
         "gdrr_destroy_volume": (i, [vp]),
         "gdrr_set_geometry": (i, [vp, d, d, d, i, i, d, d, d, d, i, vp, d]),
+        "gdrr_set_geometry_poses": (i, [vp, i, i, d, d, d, d, i, vp, d]),
         "gdrr_set_spectrum": (i, [vp, i, i, vp, vp, vp, vp, vp, vp]),
         "gdrr_project": (i, [vp, vp, i, i, vp, vp, vp, vp]),
         "gdrr_project_host": (i, [vp, vp, i, i, vp, vp, i, vp]),
@@ -223,6 +225,13 @@ def gdrr_set_geometry(ctx, sad_mm, sdd_mm, theta_rad, nu, nv, du_mm, dv_mm, u_of
                                   float(v_offset_mm), int(phi.shape[0]), phi_p, float(step_mm)), ctx)
 
 
+def gdrr_set_geometry_poses(ctx, nu, nv, du_mm, dv_mm, u_offset_mm, v_offset_mm, poses, step_mm):
+    """poses: float64 [n_proj][12] = per projection source S, detector origin P, u_hat, v_hat (mm)."""
+    ps, ps_p = _host(np.ascontiguousarray(poses, dtype=np.float64).reshape(-1, 12), np.float64)
+    _check(_lib.gdrr_set_geometry_poses(ctx, int(nu), int(nv), float(du_mm), float(dv_mm), float(u_offset_mm),
+                                        float(v_offset_mm), int(ps.shape[0]), ps_p, float(step_mm)), ctx)
+
+
 def gdrr_set_spectrum(ctx, phi_weight, response, mu_hat, fluence_map=None, bowtie_mu=None,
                       bowtie_thickness_mm=None):
     mu, mu_p = _host(mu_hat, np.float64)
@@ -315,8 +324,11 @@ class Projector:
         self.method = method
         gdrr_set_method(self.ctx, method)
         gdrr_set_sampler(self.ctx, sampler)
-        gdrr_set_geometry(self.ctx, w.sad, w.sdd, w.theta, w.nu, w.nv, w.du, w.dv, w.u_off, w.v_off,
-                          w.phis, w.step_mm)
+        if getattr(w, "poses", None) is not None:      # helical / C-arm / free source path
+            gdrr_set_geometry_poses(self.ctx, w.nu, w.nv, w.du, w.dv, w.u_off, w.v_off, w.poses, w.step_mm)
+        else:
+            gdrr_set_geometry(self.ctx, w.sad, w.sdd, w.theta, w.nu, w.nv, w.du, w.dv, w.u_off, w.v_off,
+                              w.phis, w.step_mm)
         gdrr_set_spectrum(self.ctx, w.phi_weight, w.response, w.mu_hat, w.fluence_map, w.bowtie_mu,
                           w.bowtie_thickness)
         nx, ny, nz = w.dims

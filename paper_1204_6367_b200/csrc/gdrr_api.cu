@@ -25,10 +25,10 @@ struct gdrr_context {
     unsigned long long launches = 0;
     // geometry
     bool has_geom = false;
-    double sad = 0, sdd = 0, theta = 0, du = 0, dv = 0, u_off = 0, v_off = 0, step = 0;
+    double du = 0, dv = 0, u_off = 0, v_off = 0, step = 0;
     int nu = 0, nv = 0, n_proj = 0;
-    std::vector<double> phi;
-    double4* angles_dev = nullptr;
+    std::vector<double> poses;      // [n_proj][12] source S, detector origin P, u_hat, v_hat
+    double* poses_dev = nullptr;
     // spectrum
     bool has_spec = false;
     int n_energy = 0, n_mat = 0;
@@ -172,8 +172,6 @@ int fill_geom(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int pro
                     proj_begin, proj_count, ctx->n_proj);
     if (proj_count > 65535)
         return fail(ctx, GDRR_ERR_UNSUPPORTED, "at most 65535 projections per call (got %d)", proj_count);
-    g.sad = ctx->sad;
-    g.aid = ctx->sdd - ctx->sad;
     g.half_nu = 0.5 * (double)(ctx->nu - 1);
     g.half_nv = 0.5 * (double)(ctx->nv - 1);
     g.du = ctx->du; g.dv = ctx->dv; g.u_off = ctx->u_off; g.v_off = ctx->v_off;
@@ -189,12 +187,12 @@ int fill_geom(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int pro
         if (vol->d[a] < dmin) dmin = vol->d[a];
     }
     g.step = ctx->step > 0.0 ? ctx->step : 0.5 * dmin;       // PAPER.md:155, reading Q8
-    g.angles = ctx->angles_dev;
+    g.poses = ctx->poses_dev;
     g.nu = ctx->nu; g.nv = ctx->nv;
     g.proj_begin = proj_begin; g.proj_count = proj_count;
     // the source must be outside the volume box for every requested angle
     for (int p = proj_begin; p < proj_begin + proj_count; ++p) {
-        const double S[3] = {-(ctx->sad * std::cos(ctx->phi[p])), -(ctx->sad * std::sin(ctx->phi[p])), 0.0};
+        const double* S = &ctx->poses[12 * (size_t)p];
         bool inside = true;
         for (int a = 0; a < 3; ++a) inside = inside && S[a] >= g.lo[a] && S[a] <= g.hi[a];
         if (inside)
@@ -286,6 +284,33 @@ cudaError_t ensure_compact(const gdrr_volume* vol, cudaStream_t s) {
     return e;
 }
 
+// Extent, in voxels per axis, of the beam of a 16 x 16-pixel CTA over 16 steps at the depth of the box
+// centre, the largest over the requested projections: does it fit the staged sampler's box?  (Thresholds
+// measured on C1-C4 over all gantry angles; the beam's divergence across the volume is in their margin.)
+bool beam_fits(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& g) {
+    double ext[3] = {0.0, 0.0, 0.0};
+    for (int p = g.proj_begin; p < g.proj_begin + g.proj_count; ++p) {
+        const double* q = &c->poses[12 * (size_t)p];
+        const double *S = q, *P = q + 3, *uh = q + 6, *vh = q + 9;
+        const double nrm[3] = {uh[1] * vh[2] - uh[2] * vh[1], uh[2] * vh[0] - uh[0] * vh[2], uh[0] * vh[1] - uh[1] * vh[0]};
+        double sp = 0.0, sc = 0.0, sdd = 0.0, nn = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            sp += (P[a] - S[a]) * (P[a] - S[a]);
+            sc += (vol->c[a] - S[a]) * (vol->c[a] - S[a]);
+            sdd += (P[a] - S[a]) * nrm[a];
+            nn += nrm[a] * nrm[a];
+        }
+        sdd = std::fabs(sdd) / std::sqrt(nn);
+        const double mag = std::sqrt(sc) / sdd;
+        for (int a = 0; a < 3; ++a) {
+            const double e = (16.0 * mag * (g.du * std::fabs(uh[a]) + g.dv * std::fabs(vh[a])) +
+                              16.0 * g.step * std::fabs(P[a] - S[a]) / std::sqrt(sp)) / vol->d[a];
+            ext[a] = std::fmax(ext[a], e);
+        }
+    }
+    return ext[0] <= 12.5 && ext[1] <= 12.5 && ext[2] <= 9.0;
+}
+
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
     if (vol->ctx->method == GDRR_METHOD_SIDDON) {
         cudaError_t e = ensure_compact(vol, s);
@@ -297,11 +322,7 @@ cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaS
         // AUTO: staging pays when the beam of a 16 x 16-pixel CTA over 16 steps fits the 14 x 14 x 11-quad box
         // (a chunk that does not fit is gathered anyway, after paying for its bounding box)
         const gdrr_context* c = vol->ctx;
-        const double mag = c->sad / c->sdd;
-        const double fu = 16.0 * c->du * mag / std::fmin(vol->d[0], vol->d[1]);
-        const double fv = 16.0 * c->dv * mag / vol->d[2];
-        const double adv = 16.0 * P.g.step / std::fmin(vol->d[0], vol->d[1]);
-        const bool fits = fu <= 10.0 && fv <= 8.5 && adv <= 9.0;
+        const bool fits = beam_fits(c, vol, P.g);
         // (the staged kernel walks chunks of 16 steps: P.chunk < 16 means 16 steps would overflow the 9.23 fixed point)
         if (P.chunk >= 16 && (fits || c->sampler == GDRR_SAMPLER_STAGED)) return launch_project_staged(P, vol->vw, &vol->tmap, s);
     }
@@ -337,7 +358,7 @@ int gdrr_create_context(int cuda_device, gdrr_context** out) {
 int gdrr_destroy_context(gdrr_context* ctx) {
     if (!ctx) return GDRR_OK;
     DeviceGuard guard(ctx->device);
-    free_dev(ctx->angles_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
+    free_dev(ctx->poses_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
     free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->flag_dev);
     for (int k = 0; k < 2; ++k) {
         if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
@@ -461,6 +482,31 @@ int gdrr_destroy_volume(gdrr_volume* vol) {
     return GDRR_OK;
 }
 
+// Installs a detector and a pose table (12 doubles per projection) as the context's geometry.
+static int install_geometry(gdrr_context* ctx, int nu, int nv, double du_mm, double dv_mm, double u_offset_mm,
+                            double v_offset_mm, int n_proj, std::vector<double>&& poses, double step_mm) {
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    double* dev = nullptr;
+    cudaError_t e = cudaMalloc(&dev, sizeof(double) * poses.size());
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMalloc(poses)");
+    e = cudaMemcpy(dev, poses.data(), sizeof(double) * poses.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(dev); return cuda_fail(ctx, e, "cudaMemcpy(poses)"); }
+    if (ctx->has_geom && (nu != ctx->nu || nv != ctx->nv)) {
+        // tables shaped by the old detector are no longer valid
+        free_dev(ctx->flu_dev); free_dev(ctx->bt_dev);
+        ctx->has_spec = false;
+    }
+    free_dev(ctx->poses_dev);
+    ctx->poses_dev = dev;
+    ctx->poses = std::move(poses);
+    ctx->nu = nu; ctx->nv = nv; ctx->du = du_mm; ctx->dv = dv_mm;
+    ctx->u_off = u_offset_mm; ctx->v_off = v_offset_mm;
+    ctx->n_proj = n_proj; ctx->step = step_mm;
+    ctx->has_geom = true;
+    return GDRR_OK;
+}
+
 int gdrr_set_geometry(gdrr_context* ctx, double sad_mm, double sdd_mm, double theta_rad,
                       int nu, int nv, double du_mm, double dv_mm, double u_offset_mm, double v_offset_mm,
                       int n_proj, const double* phi_rad, double step_mm) {
@@ -474,33 +520,43 @@ int gdrr_set_geometry(gdrr_context* ctx, double sad_mm, double sdd_mm, double th
     if (n_proj <= 0 || !phi_rad) return fail(ctx, GDRR_ERR_INVALID_ARG, "need n_proj >= 1 and phi_rad");
     if (!all_finite(phi_rad, (size_t)n_proj)) return fail(ctx, GDRR_ERR_INVALID_ARG, "a gantry angle is not finite");
 
-    DeviceGuard guard(ctx->device);
-    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
-    // cos/sin once, on the host, passed to the kernels as data (DESIGN.md a1)
-    std::vector<double4> ang((size_t)n_proj);
+    // cos/sin once, on the host; S, P, u_hat formed here in the order DESIGN.md a1 writes (plain IEEE
+    // double products, this file is compiled without FMA contraction) and passed to the kernels as data
+    std::vector<double> poses(12 * (size_t)n_proj, 0.0);
+    const double aid = sdd_mm - sad_mm;
     for (int p = 0; p < n_proj; ++p) {
         const double phi = phi_rad[p], psi = phi + theta_rad;
-        ang[p] = make_double4(std::cos(phi), std::sin(phi), std::cos(psi), std::sin(psi));
+        const double c = std::cos(phi), sn = std::sin(phi), cp = std::cos(psi), sp = std::sin(psi);
+        double* q = &poses[12 * (size_t)p];
+        q[0] = -(sad_mm * c); q[1] = -(sad_mm * sn); q[2] = 0.0;      // source on the circle of radius SAD  [Q1]
+        q[3] = aid * cp;      q[4] = aid * sp;       q[5] = 0.0;      // detector origin P = AID * n_hat     [Q2]
+        q[6] = -sp;           q[7] = cp;             q[8] = 0.0;      // u_hat = z_hat x n_hat               [Q3]
+        q[9] = 0.0;           q[10] = 0.0;           q[11] = 1.0;     // v_hat = +z
     }
-    double4* dev = nullptr;
-    cudaError_t e = cudaMalloc(&dev, sizeof(double4) * (size_t)n_proj);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMalloc(angles)");
-    e = cudaMemcpy(dev, ang.data(), sizeof(double4) * (size_t)n_proj, cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) { cudaFree(dev); return cuda_fail(ctx, e, "cudaMemcpy(angles)"); }
-    if (ctx->has_geom && (nu != ctx->nu || nv != ctx->nv)) {
-        // tables shaped by the old detector are no longer valid
-        free_dev(ctx->flu_dev); free_dev(ctx->bt_dev);
-        ctx->has_spec = false;
+    return install_geometry(ctx, nu, nv, du_mm, dv_mm, u_offset_mm, v_offset_mm, n_proj, std::move(poses), step_mm);
+}
+
+int gdrr_set_geometry_poses(gdrr_context* ctx, int nu, int nv, double du_mm, double dv_mm,
+                            double u_offset_mm, double v_offset_mm, int n_proj, const double* poses,
+                            double step_mm) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    const double sc[] = {du_mm, dv_mm, u_offset_mm, v_offset_mm, step_mm};
+    if (!all_finite(sc, 5)) return fail(ctx, GDRR_ERR_INVALID_ARG, "a geometry scalar is not finite");
+    if (nu <= 0 || nv <= 0 || !(du_mm > 0) || !(dv_mm > 0))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "detector pixel counts and sizes must be positive");
+    if (n_proj <= 0 || !poses) return fail(ctx, GDRR_ERR_INVALID_ARG, "need n_proj >= 1 and poses");
+    if (!all_finite(poses, 12 * (size_t)n_proj)) return fail(ctx, GDRR_ERR_INVALID_ARG, "a pose value is not finite");
+    for (int p = 0; p < n_proj; ++p) {
+        const double* q = poses + 12 * (size_t)p;
+        const double *S = q, *P = q + 3, *uh = q + 6, *vh = q + 9;
+        const double nrm[3] = {uh[1] * vh[2] - uh[2] * vh[1], uh[2] * vh[0] - uh[0] * vh[2], uh[0] * vh[1] - uh[1] * vh[0]};
+        const double nn = nrm[0] * nrm[0] + nrm[1] * nrm[1] + nrm[2] * nrm[2];
+        const double dist = (P[0] - S[0]) * nrm[0] + (P[1] - S[1]) * nrm[1] + (P[2] - S[2]) * nrm[2];
+        if (!(nn > 0.0)) return fail(ctx, GDRR_ERR_INVALID_ARG, "projection %d: u_hat and v_hat do not span a plane", p);
+        if (dist == 0.0) return fail(ctx, GDRR_ERR_INVALID_ARG, "projection %d: the source lies in the detector plane", p);
     }
-    free_dev(ctx->angles_dev);
-    ctx->angles_dev = dev;
-    ctx->sad = sad_mm; ctx->sdd = sdd_mm; ctx->theta = theta_rad;
-    ctx->nu = nu; ctx->nv = nv; ctx->du = du_mm; ctx->dv = dv_mm;
-    ctx->u_off = u_offset_mm; ctx->v_off = v_offset_mm;
-    ctx->n_proj = n_proj; ctx->step = step_mm;
-    ctx->phi.assign(phi_rad, phi_rad + n_proj);
-    ctx->has_geom = true;
-    return GDRR_OK;
+    std::vector<double> copy(poses, poses + 12 * (size_t)n_proj);
+    return install_geometry(ctx, nu, nv, du_mm, dv_mm, u_offset_mm, v_offset_mm, n_proj, std::move(copy), step_mm);
 }
 
 int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,

@@ -17,14 +17,13 @@ constexpr int kFracBits = 23;       // fixed-point fraction bits of the in-chunk
 // Everything the ray-setup arithmetic (step a1) needs.  All fp64; the order of
 // operations in ray_setup.cuh is part of the definition of (j0, n).
 struct GeomParams {
-    double sad, aid;                // source-to-axis, axis-to-imager (= sdd - sad)
     double half_nu, half_nv;        // 0.5 * (nu - 1), 0.5 * (nv - 1)
     double du, dv, u_off, v_off;
     double step;                    // dl
     double lo[3], hi[3];            // volume box
     double c[3], d[3];              // box centre, voxel size
     double ofs[3];                  // 0.5 * (N - 1) + 1: world -> padded index coordinates
-    const double4* angles;          // [n_proj] (cos phi, sin phi, cos psi, sin psi), device
+    const double* poses;            // [n_proj][12] source S, detector origin P, u_hat, v_hat; device
     int nu, nv;
     int proj_begin, proj_count;
 };

@@ -4,7 +4,8 @@
 // bit for bit with the CPU oracle, so every operation that feeds it is an
 // explicitly rounded IEEE-754 double operation (__dadd_rn, __dmul_rn, __ddiv_rn,
 // __dsqrt_rn: never contracted into an FMA) in the order DESIGN.md "a1" writes
-// out.  cos/sin of the angles arrive as data (taken once on the host).
+// out.  Source and detector frame arrive as data (for the gantry: cos/sin taken
+// once on the host, products formed there in the oracle's order).
 #pragma once
 #include "gdrr_internal.h"
 
@@ -19,20 +20,21 @@ struct Ray {
 };
 
 __device__ __forceinline__ void ray_setup(const GeomParams& g, int p, int i, int j, Ray& r) {
-    const double4 a = g.angles[p];                 // (cos phi, sin phi, cos psi, sin psi)
-    // detector origin P = AID * n_hat; u_hat = z_hat x n_hat; v_hat = +z  [Q2][Q3]
-    const double Px = __dmul_rn(g.aid, a.z), Py = __dmul_rn(g.aid, a.w);
-    const double ux = -a.w, uy = a.z;
-    // source on the circle of radius SAD  [Q1]
-    r.S[0] = -__dmul_rn(g.sad, a.x);
-    r.S[1] = -__dmul_rn(g.sad, a.y);
-    r.S[2] = 0.0;
-    // one ray through the pixel centre  [Q4][Q5]
+    // the pose of projection p: source S, detector origin P, u_hat, v_hat (12 doubles).  For the
+    // circular gantry the host fills it from (SAD, SDD, phi, theta) [Q1][Q2][Q3]; helical and C-arm
+    // source paths give it directly [Q31]
+    const double* pose = g.poses + 12 * (size_t)p;
+    // one ray through the pixel centre D = (P + u u_hat) + v v_hat  [Q4][Q5]
     const double u = __dadd_rn(__dmul_rn(__dsub_rn((double)i, g.half_nu), g.du), g.u_off);
     const double v = __dadd_rn(__dmul_rn(__dsub_rn((double)j, g.half_nv), g.dv), g.v_off);
-    const double D0 = __dadd_rn(Px, __dmul_rn(u, ux));
-    const double D1 = __dadd_rn(Py, __dmul_rn(u, uy));
-    const double dx = __dsub_rn(D0, r.S[0]), dy = __dsub_rn(D1, r.S[1]), dz = __dsub_rn(v, r.S[2]);
+    double D[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        r.S[k] = pose[k];
+        D[k] = __dadd_rn(__dadd_rn(pose[3 + k], __dmul_rn(u, pose[6 + k])), __dmul_rn(v, pose[9 + k]));
+    }
+    const double D0 = D[0], D1 = D[1];
+    const double dx = __dsub_rn(D0, r.S[0]), dy = __dsub_rn(D1, r.S[1]), dz = __dsub_rn(D[2], r.S[2]);
     const double L = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)),
                                           __dmul_rn(dz, dz)));
     r.dir[0] = __ddiv_rn(dx, L);
