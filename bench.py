@@ -208,6 +208,12 @@ def run_b200(args):
         w = w0.with_phis(gd.scan_angles(n_total)[mine])
     else:                                                   # profiling aid: every projection at one angle
         w = w0.with_phis(np.full(per_gpu, np.deg2rad(args.angle_deg)))
+    if args.trajectory != "circle":                         # other source paths, same kernels
+        from workloads import trajectories
+        nz_mm = w.dims[2] * w.spacing[2]
+        w = w.with_poses(trajectories.helical_poses(w.sad, w.sdd, w.phis, pitch_mm=0.5 * nz_mm, z0_mm=-0.25 * nz_mm)
+                         if args.trajectory == "helix" else
+                         trajectories.c_arm_poses(w.sad, w.sdd, w.phis, np.deg2rad(args.tilt_deg)))
     launch_proj = per_gpu if args.launch_proj <= 0 else min(args.launch_proj, per_gpu)
 
     pr = g.Projector(w, device=local_rank, layout=args.layout,
@@ -368,7 +374,8 @@ def run_b200(args):
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
-            "config": workload_config(w, args.workload, world, n_total, launch_proj),
+            "config": dict(workload_config(w, args.workload, world, n_total, launch_proj),
+                           **({} if args.trajectory == "circle" else {"trajectory": args.trajectory})),
             "projections_per_s": proj_per_s, "samples_per_step": total_samples,
             "paper_context": "paper: 1.2-2.3 s per poly-energetic projection on a GTX 580 (PAPER.md:366-367)",
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
@@ -468,6 +475,10 @@ def main():
                     help="packed-quad sampling kernel: quads staged through shared memory by TMA (auto), or gathered through L1")
     ap.add_argument("--angle-deg", type=float, default=None,
                     help="profiling aid: all projections at this one gantry angle instead of an evenly spaced scan")
+    ap.add_argument("--trajectory", default="circle", choices=["circle", "helix", "c_arm"],
+                    help="source path: the paper's circle (the headline), a one-turn helix over half the volume's "
+                         "height, or the circle tilted about x by --tilt-deg (gdrr_set_geometry_poses)")
+    ap.add_argument("--tilt-deg", type=float, default=20.0)
     ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
