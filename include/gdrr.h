@@ -99,7 +99,7 @@ enum {
                                   CTA over 16 steps can fit the 14 x 14 x 11-quad box; else GATHER */
     GDRR_SAMPLER_GATHER = 1,   /* quads gathered from global memory through L1 */
     GDRR_SAMPLER_STAGED = 2    /* quads of a CTA's beam staged through shared memory by TMA (a chunk whose beam
-                                  does not fit is gathered; GATHER is used if 16 steps exceed 120 voxels) */
+                                  does not fit is gathered; GATHER is used if 16 steps exceed 15 voxels) */
 };
 
 #define GDRR_MAX_MATERIALS 4

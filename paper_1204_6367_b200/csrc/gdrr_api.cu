@@ -324,8 +324,9 @@ cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaS
         // (a chunk that does not fit is gathered anyway, after paying for its bounding box)
         const gdrr_context* c = vol->ctx;
         const bool fits = beam_fits(c, vol, P.g);
-        // (the staged kernel walks chunks of 16 steps: P.chunk < 16 means 16 steps would overflow the 9.23 fixed point)
-        if (P.chunk >= 16 && (fits || c->sampler == GDRR_SAMPLER_STAGED)) return launch_project_staged(P, vol->vw, &vol->tmap, s);
+        // (the staged kernel keeps a chunk's base in 5.27 fixed point: 16 steps must advance less than 16 voxels)
+        const double adv16 = 16.0 * P.g.step / std::fmin(vol->d[0], std::fmin(vol->d[1], vol->d[2]));
+        if (adv16 <= 15.0 && (fits || c->sampler == GDRR_SAMPLER_STAGED)) return launch_project_staged(P, vol->vw, &vol->tmap, s);
     }
     if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
     return launch_project_exact(P, vol->vw, vol->layout, s);

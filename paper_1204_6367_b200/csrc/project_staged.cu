@@ -30,6 +30,7 @@ constexpr int kBX = 14, kBY = 14, kBZ = 11;       // box, in quads
 constexpr int kBoxElems = kBX * kBY * kBZ;        // 2156 quads = 34,496 B
 constexpr int kStageElems = 2160;                 // stage pitch: 34,560 B, a multiple of 128
 constexpr unsigned kBoxBytes = kBoxElems * 16u;
+constexpr int kBaseBits = 27;                     // fraction bits of a chunk's base position (5.27 fixed point)
 
 __device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -150,7 +151,7 @@ __device__ __forceinline__ void run_chunk_staged_pairs(const Sampler& S, int qx,
 struct StageCtl {
     unsigned long long bar[2];     // "box of stage s has landed"
     int bb[3][6];                  // bounding box of chunk m in bb[m % 3]: min x, y, z, max x, y, z (cells)
-    int org[2][3];                 // origin of the box in stage s
+    int lin[2];                    // stage s: element of cell (cx, cy, cz) = lin + (cz kBY + cy) kBX + cx
     int fit[2];                    // stage s holds the box of its chunk (else: gather from global memory)
     int krange[2];                 // smallest first / largest last+1 interval index of the CTA's rays
 };
@@ -233,27 +234,35 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
         const int c_begin = kmin / kStageK;
         const int nchunks = (kmax - 1) / kStageK - c_begin + 1;
 
-        // base position of chunk m, and this ray's share of the chunk's bounding box -> ctl.bb[m % 3]
-        // (every 4th chunk the base is re-formed in fp64; in between it is the previous base advanced by
-        // kStageK steps in the loop's own fixed-point arithmetic: drift <= 64 * 2^-24 voxel)
-        auto prepare = [&](int m, int slot, ChunkBase& b) {
-            const int kc = (c_begin + m) * kStageK;
-            if ((m & 3) == 0) {
-                b = chunk_base(gs, dg, kc);
-            } else {
-                const int qx = b.qx + kStageK * S.dqx, qy = b.qy + kStageK * S.dqy, qz = b.qz + kStageK * S.dqz;
-                b.cx += qx >> kFracBits; b.cy += qy >> kFracBits; b.cz += qz >> kFracBits;
-                b.qx = qx & ((1 << kFracBits) - 1); b.qy = qy & ((1 << kFracBits) - 1); b.qz = qz & ((1 << kFracBits) - 1);
+        // Chunk bases.  The position of a chunk's first sample is (cell cb, fraction qb in 2^-27 voxel); the
+        // next chunk's is that plus D = round(kStageK dg 2^27), in integers.  The fp64 line of the ray is used
+        // once, for chunk 0: the base then drifts by <= 2^-28 voxel per chunk (2^-19 over the 500 chunks of
+        // the longest ray a 180 GB volume allows), and 12 registers of doubles do not live through the loop.
+        // Inside a chunk the samples step by dq = round(dg 2^23) from the base's 23-bit fraction.
+        int cb[3], qb[3], D[3];
+        {
+            const double tk = (double)(c_begin * kStageK) + 0.5;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const double x = fma(tk, dg[a], gs[a]);
+                const double f = floor(x);
+                cb[a] = (int)f;
+                qb[a] = (int)((x - f) * (double)(1 << kBaseBits));
+                D[a] = __double2int_rn(dg[a] * (double)kStageK * (double)(1 << kBaseBits));
             }
+        }
+        // this ray's share of the bounding box of the chunk whose base is (cb, qb), first index kc -> ctl.bb[slot]
+        auto contribute = [&](int kc, int slot) {
             const int lo = max(j0 - kc, 0), hi = min(j0 + n - kc, kStageK);
             int mn[3] = {0x7fffffff, 0x7fffffff, 0x7fffffff};
             int mx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
             if (hi > lo) {                       // cells of the first and the last sample, exactly as the loop forms them
-                const int bc[3] = {b.cx, b.cy, b.cz}, bq[3] = {b.qx, b.qy, b.qz}, dq[3] = {S.dqx, S.dqy, S.dqz};
+                const int dq[3] = {S.dqx, S.dqy, S.dqz};
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
-                    const int c_lo = bc[a] + ((bq[a] + lo * dq[a]) >> kFracBits);
-                    const int c_hi = bc[a] + ((bq[a] + (hi - 1) * dq[a]) >> kFracBits);
+                    const int q23 = qb[a] >> (kBaseBits - kFracBits);
+                    const int c_lo = cb[a] + ((q23 + lo * dq[a]) >> kFracBits);
+                    const int c_hi = cb[a] + ((q23 + (hi - 1) * dq[a]) >> kFracBits);
                     mn[a] = min(c_lo, c_hi);
                     mx[a] = max(c_lo, c_hi);
                 }
@@ -273,18 +282,15 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             const bool fit = bb[0] <= bb[3] && bb[3] - bb[0] + 1 <= kBX && bb[4] - bb[1] + 1 <= kBY &&
                              bb[5] - bb[2] + 2 <= kBZ;
             ctl.fit[st] = fit;
-            ctl.org[st][0] = bb[0];
-            ctl.org[st][1] = bb[1];
-            ctl.org[st][2] = bb[2];
+            // element of cell (cx, cy, cz) in the stage: lin + (cz kBY + cy) kBX + cx
+            ctl.lin[st] = st * kStageElems - ((bb[2] * kBY + bb[1]) * kBX + bb[0]);
             if (fit) {
                 mbar_arrive_expect_tx(&ctl.bar[st], kBoxBytes);
                 tma_load_box(s_box + st * kStageElems, &tmap, 4 * bb[0], bb[1], bb[2], &ctl.bar[st]);
             }
         };
 
-        ChunkBase b_cur, b_next;
-        prepare(0, 0, b_cur);
-        b_next = b_cur;
+        contribute(c_begin * kStageK, 0);
         __syncthreads();
         if (threadIdx.x == 0) issue(0, 0);
         unsigned phase[2] = {0u, 0u};
@@ -295,7 +301,22 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             if (threadIdx.x == 0) {              // the slot chunk m + 2 will use: consumed two iterations ago
                 for (int a = 0; a < 3; ++a) { ctl.bb[slot2][a] = 0x7fffffff; ctl.bb[slot2][3 + a] = (int)0x80000000; }
             }
-            if (m + 1 < nchunks) prepare(m + 1, slot1, b_next);
+            // chunk m: working copy of its base; then the base moves on to chunk m + 1
+            const int kc = (c_begin + m) * kStageK;
+            const int wqx = qb[0] >> (kBaseBits - kFracBits), wqy = qb[1] >> (kBaseBits - kFracBits),
+                      wqz = qb[2] >> (kBaseBits - kFracBits);
+            const int rel_cell = (cb[2] * kBY + cb[1]) * kBX + cb[0];
+            int dc[3] = {0, 0, 0};               // cells the base advanced by (the gather fallback wants chunk m's cell)
+            if (m + 1 < nchunks) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const int q = qb[a] + D[a];
+                    dc[a] = q >> kBaseBits;
+                    cb[a] += dc[a];
+                    qb[a] = q & ((1 << kBaseBits) - 1);
+                }
+                contribute(kc + kStageK, slot1);
+            }
             __syncthreads();                     // box of m + 1 known; everyone is done with stage st ^ 1
             if (threadIdx.x == 0 && m + 1 < nchunks) issue(m + 1, slot1);
             {
@@ -304,7 +325,6 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
                 slot2 = s0;
             }
 
-            const int kc = (c_begin + m) * kStageK;
             const unsigned rel = (unsigned)(kc - j0);
             const bool mine = rel < un && rel + (unsigned)kStageK <= un;     // this lane owns the whole chunk
             const bool all_mine = __all_sync(0xffffffffu, mine);
@@ -314,19 +334,20 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             if (ctl.fit[st]) {
                 mbar_wait(&ctl.bar[st], phase[st]);
                 phase[st] ^= 1u;
-                const int idx0 = st * kStageElems + ((b_cur.cz - ctl.org[st][2]) * kBY + (b_cur.cy - ctl.org[st][1])) * kBX +
-                                 (b_cur.cx - ctl.org[st][0]);
-                if (all_mine) run_chunk_staged_pairs<VW>(S, b_cur.qx, b_cur.qy, b_cur.qz, idx0, A);
-                else run_chunk_staged<VW, true>(S, b_cur.qx, b_cur.qy, b_cur.qz, idx0, kStageK, rel, un, A);
+                const int idx0 = rel_cell + ctl.lin[st];
+                if (all_mine) run_chunk_staged_pairs<VW>(S, wqx, wqy, wqz, idx0, A);
+                else run_chunk_staged<VW, true>(S, wqx, wqy, wqz, idx0, kStageK, rel, un, A);
             } else {
-                if (all_mine) run_chunk<VW, false>(S, b_cur, kStageK, rel, un, A);
-                else run_chunk<VW, true>(S, b_cur, kStageK, rel, un, A);
+                ChunkBase b;
+                b.cx = cb[0] - dc[0]; b.cy = cb[1] - dc[1]; b.cz = cb[2] - dc[2];
+                b.qx = wqx; b.qy = wqy; b.qz = wqz;
+                if (all_mine) run_chunk<VW, false>(S, b, kStageK, rel, un, A);
+                else run_chunk<VW, true>(S, b, kStageK, rel, un, A);
             }
             add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur);
             A.cur = 0.f;
 #pragma unroll
             for (int k = 0; k < VW; ++k) acc[k] += A.part[k];
-            b_cur = b_next;
         }
     }
 
