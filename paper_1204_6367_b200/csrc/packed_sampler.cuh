@@ -54,6 +54,19 @@ __device__ __forceinline__ float frac_float(int q, unsigned mask, unsigned one) 
     return __uint_as_float(o) - 1.f;
 }
 
+// The same in two steps, for the pair loop of the staged sampler: bits of 1 + fraction, then
+// (1 + f0, 1 + f1) - (1, 1) as one packed add.
+__device__ __forceinline__ unsigned frac_bits(int q, unsigned mask, unsigned one) {
+    unsigned o;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(o) : "r"(q), "r"(mask), "r"(one));
+    return o;
+}
+__device__ __forceinline__ void sub_one2(unsigned b0, unsigned b1, float& f0, float& f1) {
+    f32x2 r;
+    asm("add.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(b0, b1)), "l"(pack2(0xBF800000u, 0xBF800000u)));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(f0), "=f"(f1) : "l"(r));
+}
+
 // thread -> pixel: a warp is 4 (u) x 8 (v) pixels, so that a load phase (8 consecutive lanes) is a
 // compact 4 x 2 patch of rays; the CTA's 16 x 16 tile is 4 x 2 warps.
 __device__ __forceinline__ void thread_pixel_map(int& i, int& j) {
