@@ -286,7 +286,7 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
         contribute(c_begin * kStageK, 0);
         __syncthreads();
         if (threadIdx.x == 0) issue(0, 0);
-        unsigned phase[2] = {0u, 0u};
+        unsigned phases = 0u;                    // bit st: parity of the next completion of bar[st]
         int slot1 = 1, slot2 = 2;                // bounding-box slots of chunks m + 1 and m + 2 (m % 3 rotation)
 
         for (int m = 0; m < nchunks; ++m) {
@@ -325,8 +325,8 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             for (int k = 0; k < VW; ++k) A.part[k] = 0.f;
 
             if (ctl.fit[st]) {
-                mbar_wait(&ctl.bar[st], phase[st]);
-                phase[st] ^= 1u;
+                mbar_wait(&ctl.bar[st], (phases >> st) & 1u);
+                phases ^= 1u << st;
                 const int idx0 = rel_cell + ctl.lin[st];
                 if (all_mine) run_chunk_staged_pairs<VW>(S, wqx, wqy, wqz, idx0, A);
                 else run_chunk_staged<VW, true>(S, wqx, wqy, wqz, idx0, kStageK, rel, un, A);
