@@ -263,7 +263,7 @@ bool make_tensor_map(gdrr_volume* v) {
     }
     const cuuint64_t dims[3] = {4ull * (cuuint64_t)v->px, (cuuint64_t)v->py, (cuuint64_t)v->pz};
     const cuuint64_t strides[2] = {16ull * (cuuint64_t)v->sy, 16ull * (cuuint64_t)v->sz};      // bytes, dims 1 and 2
-    const cuuint32_t box[3] = {56u, 14u, 11u};
+    const cuuint32_t box[3] = {4u * kBX, (cuuint32_t)kBY, (cuuint32_t)kBZ};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     CUresult r = ((encode_fn)fn)(&v->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, v->vox, dims, strides, box, estr,
                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,

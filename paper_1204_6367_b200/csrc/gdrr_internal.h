@@ -11,6 +11,16 @@ namespace gdrr {
 constexpr int kTileU = 16;
 constexpr int kTileV = 16;
 constexpr int kThreads = kTileU * kTileV;
+// staged sampler: its own CTA tile and staging box (project_staged.cu; the tensor map is made in gdrr_api.cu)
+// (measured on C3: a 16 x 8 tile with a 14 x 14 x 7 box, 4 CTAs per SM: -8%)
+#ifndef GDRR_STAGE_TILE_V
+#define GDRR_STAGE_TILE_V 16
+#define GDRR_STAGE_BOX_Z 11
+#define GDRR_STAGE_CTAS 3
+#endif
+constexpr int kStageTileV = GDRR_STAGE_TILE_V;
+constexpr int kStageThreads = kTileU * kStageTileV;
+constexpr int kBX = 14, kBY = 14, kBZ = GDRR_STAGE_BOX_Z;       // box, in quads
 constexpr int kMaxChunk = 32;       // samples between two fp64 re-bases of the position
 constexpr int kFracBits = 23;       // fixed-point fraction bits of the in-chunk position
 

@@ -26,9 +26,8 @@
 namespace gdrr {
 
 constexpr int kStageK = 16;                       // interval indices per staged chunk
-constexpr int kBX = 14, kBY = 14, kBZ = 11;       // box, in quads
 constexpr int kBoxElems = kBX * kBY * kBZ;        // 2156 quads = 34,496 B
-constexpr int kStageElems = 2160;                 // stage pitch: 34,560 B, a multiple of 128
+constexpr int kStageElems = (kBoxElems + 7) / 8 * 8;  // stage pitch: a multiple of 128 B
 constexpr unsigned kBoxBytes = kBoxElems * 16u;
 constexpr int kBaseBits = 27;                     // fraction bits of a chunk's base position (5.27 fixed point)
 
@@ -150,12 +149,12 @@ struct StageCtl {
 };
 
 template <int VW>
-__global__ void __launch_bounds__(kThreads, 3)
+__global__ void __launch_bounds__(kStageThreads, GDRR_STAGE_CTAS)
 gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtensorMap tmap) {
     __shared__ StageCtl ctl;
     float4* s_mu = reinterpret_cast<float4*>(s_box + 2 * kStageElems);
     float2* s_src = reinterpret_cast<float2*>(s_mu + P.n_energy);
-    for (int e = threadIdx.x; e < P.n_energy; e += kThreads) {
+    for (int e = threadIdx.x; e < P.n_energy; e += kStageThreads) {
         s_mu[e] = P.mu_tab[e];
         s_src[e] = P.src_tab[e];
     }
@@ -171,10 +170,11 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
     }
     __syncthreads();
 
-    int i, j;
-    thread_pixel_map(i, j);
-    const int pl = blockIdx.z;
+    // a warp is 4 (u) x 8 (v) pixels (thread_pixel_map), the CTA's tile kTileU x kStageTileV
     const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * kTileU + ((threadIdx.x >> 5) & 3) * 4 + (lane & 3);
+    const int j = blockIdx.y * kStageTileV + (threadIdx.x >> 7) * 8 + (lane >> 2);
+    const int pl = blockIdx.z;
     const bool valid = i < P.g.nu && j < P.g.nv;
 
     // ---- a1: ray setup (fp64) ------------------------------------------------
@@ -349,13 +349,13 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
 
 template <int VW>
 static cudaError_t launch_staged_t(const ProjectParams& p, const CUtensorMap& map, cudaStream_t s) {
-    dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kTileV - 1) / kTileV, p.g.proj_count);
+    dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kStageTileV - 1) / kStageTileV, p.g.proj_count);
     const size_t smem = 2 * (size_t)kStageElems * 16 + (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
     // per device and cheap: set at every launch (the boxes alone exceed the 48 KB default)
     cudaError_t e = cudaFuncSetAttribute(gdrr_project_staged_kernel<VW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          2 * kStageElems * 16 + 512 * 24 /* GDRR_MAX_ENERGIES bins */);
     if (e != cudaSuccess) return e;
-    gdrr_project_staged_kernel<VW><<<grid, kThreads, smem, s>>>(p, map);
+    gdrr_project_staged_kernel<VW><<<grid, kStageThreads, smem, s>>>(p, map);
     return cudaGetLastError();
 }
 
