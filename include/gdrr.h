@@ -118,7 +118,7 @@ GDRR_API const char* gdrr_last_error(const gdrr_context* ctx);
 /* ---- volume: step a0, PAPER.md:97 -------------------------------------- */
 
 /* Bytes of device workspace gdrr_create_volume needs for this shape (PACKED_QUAD: 16 B per quad with the
- * skewed strides, rounded to 256, plus 4 B per voxel in 128-byte bricks for the Siddon walk's compact copy). */
+ * skewed strides, rounded to 256, plus 4 B per voxel, rows padded to groups of four, for the Siddon walk's compact copy). */
 GDRR_API int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int layout,
                                 size_t* bytes);
 
@@ -230,7 +230,7 @@ GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int pr
  * line integral of its material; the energy sum, the outputs and the ray table
  * (which stays the midpoint table of the geometry) are unchanged.  A ray that
  * lies IN a lattice plane belongs to either neighbour (a tie).  Works on every
- * layout (a PACKED_QUAD workspace carries a compact bricked copy for this walk).
+ * layout (a PACKED_QUAD workspace carries a compact one-word-per-voxel copy for this walk).
  * Errors: INVALID_ARG (unknown method). */
 GDRR_API int gdrr_set_method(gdrr_context* ctx, int method);
 

@@ -126,8 +126,8 @@ size_t packed_elements(int nx, int ny, int nz) {
 }
 
 // bytes of the 4 x 4 x 2-bricked one-word-per-voxel copy kept behind the quads (Siddon walk)
-size_t compact_bytes(int nx, int ny, int nz) {
-    return (size_t)((nx + 3) / 4) * ((ny + 3) / 4) * ((nz + 1) / 2) * 128;
+size_t compact_bytes(int nx, int ny, int nz) {        // rows in groups of four, 4 B per voxel
+    return (size_t)nx * (size_t)(4 * ((ny + 3) / 4)) * (size_t)nz * 4;
 }
 
 size_t element_bytes(int n_mat, int layout) {
@@ -214,8 +214,8 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     P.v.nvox[0] = vol->nx; P.v.nvox[1] = vol->ny; P.v.nvox[2] = vol->nz;
     P.seg_table = nullptr;
     P.v.compact = vol->compact;
-    P.v.cstride_y = 32 * ((vol->nx + 3) / 4);
-    P.v.cstride_z = 32 * ((vol->nx + 3) / 4) * ((vol->ny + 3) / 4);
+    P.v.cstride_y = 4 * vol->nx;
+    P.v.cstride_z = 4 * vol->nx * ((vol->ny + 3) / 4);
     if (vol->layout == GDRR_LAYOUT_BRICK) {
         P.v.stride_y = 8 * (vol->px / 2);
         P.v.stride_z = 8 * (vol->px / 2) * (vol->py / 2);

@@ -43,8 +43,8 @@ struct VolumeParams {
     const void* vox1;               // PACKED_QUAD: vox + one slab (its own parameter: one IMAD.WIDE per load)
     int stride_y;                   // BRICK: 8 * bricks per row;   LINEAR: stored nx;      PACKED_QUAD: elements per row (= 3 mod 8)
     int nvox[3];                    // nx, ny, nz (Siddon traversal)
-    const void* compact;            // PACKED_QUAD: one tagged word per voxel in 4 x 4 x 2 bricks of 128 B (Siddon walk)
-    int cstride_y, cstride_z;       //   words per row of bricks, per slab of bricks
+    const void* compact;            // PACKED_QUAD: one tagged word per voxel, rows in groups of four (Siddon walk)
+    int cstride_y, cstride_z;       //   words per group of four rows (4 nx), per slab
     int stride_z;                   // BRICK: 8 * bricks per slab;  LINEAR: stored nx * ny; PACKED_QUAD: elements per slab (= 4 mod 8)
 };
 
@@ -71,15 +71,15 @@ struct IngestParams {
     int nx, ny, nz;
     int px, py, pz;                 // stored dims (voxels for BRICK / LINEAR, quads for PACKED_QUAD)
     int sy, sz;                     // PACKED_QUAD: element strides (VolumeParams)
-    void* compact;                  // PACKED_QUAD: the 4 x 4 x 2-bricked one-word-per-voxel copy
-    int cbx, cby;                   //   bricks per row, rows of bricks per slab
+    void* compact;                  // PACKED_QUAD: the one-word-per-voxel copy, rows in groups of four
+    int cbx, cby;                   //   ceil(nx / 4), ceil(ny / 4) (cby: groups of four rows per slab)
     int n_mat;
     int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
 };
 
 // Host-callable launchers (each returns the cudaGetLastError() of its launch).
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s);
-// PACKED_QUAD: fills p.compact (4 x 4 x 2-bricked words) from the quads in p.vox; needs nx..nz, sy, sz, cbx, cby, n_mat
+// PACKED_QUAD: fills p.compact (one word per voxel, rows in groups of four) from the quads in p.vox; needs nx..nz, sy, sz, cbx, cby, n_mat
 cudaError_t launch_compact_copy(const IngestParams& p, cudaStream_t s);
 cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);

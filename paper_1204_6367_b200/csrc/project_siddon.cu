@@ -14,7 +14,7 @@
 //
 // Works on every device layout: the exact ones hold VW floats per voxel (one per material),
 // a PACKED_QUAD volume carries a second, compact copy for this walk: the same tagged word per
-// voxel in 4 x 4 x 2 bricks of 128 B (4 B per voxel instead of 16, ~4 voxels of any walk per line).
+// voxel, rows in groups of four (4 B per voxel instead of 16; a 128-byte line is 8 x 4 voxels).
 // fp32 accumulation is chunked like the tri-linear sampler's (32 segments per partial sum).
 #include "project_common.cuh"
 
@@ -45,14 +45,14 @@ __device__ __forceinline__ void add_routed_s(float (&part)[VW], int m, float v) 
 
 // Element offset contributed by voxel index i along one axis.  LAYOUT 0: padded 2x2x2 bricks of the exact
 // BRICK layout (project_fused.cu has the same map); 1: padded linear; 2: the packed volume's compact copy,
-// unpadded bricks of 4 (x) x 4 (y) x 2 (z) words (volume_layout.cu).
+// unpadded, rows in groups of four: iz SZ + (iy >> 2) SY + 4 ix + (iy & 3) (volume_layout.cu).
 template <int LAYOUT, int AXIS>
 __device__ __forceinline__ int siddon_axis_offset(int i, int stride) {
     if (LAYOUT == 0) return ((i + 1) >> 1) * stride + (((i + 1) & 1) << AXIS);
     if (LAYOUT == 1) return (i + 1) * stride;
-    if (AXIS == 0) return (i >> 2) * 32 + (i & 3);
-    if (AXIS == 1) return (i >> 2) * stride + ((i & 3) << 2);
-    return (i >> 1) * stride + ((i & 1) << 4);
+    if (AXIS == 0) return 4 * i;
+    if (AXIS == 1) return (i >> 2) * stride + (i & 3);
+    return i * stride;
 }
 
 // len x voxel value into the per-material sums.  Exact layouts: one FMA per material.  Packed word:
@@ -84,7 +84,7 @@ __device__ __forceinline__ typename SiddonVoxel<VW, LAYOUT>::T load_voxel(const 
     return __ldg(reinterpret_cast<const T*>(vox) + off);
 }
 
-// LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed volume's compact bricked words
+// LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed volume's compact copy (one word per voxel)
 // COUNT: also count the segments of positive length (gdrr_siddon_segments)
 template <int VW, int LAYOUT, bool COUNT>
 __global__ void __launch_bounds__(kThreads)
@@ -145,7 +145,8 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
         int off = siddon_axis_offset<LAYOUT, 0>(idx[0], sx) + siddon_axis_offset<LAYOUT, 1>(idx[1], sy) +
                   siddon_axis_offset<LAYOUT, 2>(idx[2], sz);
         // linear element orders: stepping one voxel along an axis adds a constant to the element offset
-        const int dox = stp[0] * sx, doy = stp[1] * sy, doz = stp[2] * sz;
+        const int dox = stp[0] * (LAYOUT == 2 ? 4 : sx), doy = stp[1] * sy, doz = stp[2] * sz;
+        const int y_edge = stp[1] > 0 ? 3 : 0, doy_cross = stp[1] * (sy - 3);       // LAYOUT 2 only
         float kx = 0.f, ky = 0.f, kz = 0.f;              // planes crossed so far per axis (exact in fp32)
         float tx = t0[0], ty = t0[1], tz = t0[2];
         float t = 0.f;
@@ -167,20 +168,31 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
                 // cross the plane that was met (x before y before z at ties), branch-free
                 const bool bx = tx <= ty && tx <= tz;
                 const bool by = !bx && ty <= tz;
-                if (LAYOUT != 1) {
+                if (LAYOUT == 0) {
                     idx[0] += bx ? stp[0] : 0;
                     idx[1] += by ? stp[1] : 0;
                     idx[2] += (bx || by) ? 0 : stp[2];
-                    off = siddon_axis_offset<LAYOUT, 0>(idx[0], sx) + siddon_axis_offset<LAYOUT, 1>(idx[1], sy) +
-                          siddon_axis_offset<LAYOUT, 2>(idx[2], sz);
+                    // (past the last voxel the walk has stepped out of the lattice: keep the last valid offset)
+                    const int o = siddon_axis_offset<LAYOUT, 0>(idx[0], sx) + siddon_axis_offset<LAYOUT, 1>(idx[1], sy) +
+                                  siddon_axis_offset<LAYOUT, 2>(idx[2], sz);
+                    off = more ? o : off;
+                } else if (LAYOUT == 2) {
+                    // rows in groups of 4: a step in y moves by one word inside a group, by a row of groups across its edge
+                    const int dy_now = ((idx[1] & 3) == y_edge) ? doy_cross : stp[1];
+                    idx[1] += by ? stp[1] : 0;
+                    off += more ? (bx ? dox : (by ? dy_now : doz)) : 0;
                 } else {
-                    off += bx ? dox : (by ? doy : doz);
+                    off += more ? (bx ? dox : (by ? doy : doz)) : 0;
                 }
-                if (bx) { kx += 1.f; tx = fmaf(kx, dt[0], t0[0]); }
-                else if (by) { ky += 1.f; ty = fmaf(ky, dt[1], t0[1]); }
-                else { kz += 1.f; tz = fmaf(kz, dt[2], t0[2]); }
+                // plane counters and parameters of all three axes, without branches (only one counter moves)
+                kx += bx ? 1.f : 0.f;
+                ky += by ? 1.f : 0.f;
+                kz += (bx || by) ? 0.f : 1.f;
+                tx = fmaf(kx, dt[0], t0[0]);
+                ty = fmaf(ky, dt[1], t0[1]);
+                tz = fmaf(kz, dt[2], t0[2]);
                 const VT cv = v;
-                if (more) v = load_voxel<VW, LAYOUT>(vox, off);
+                v = load_voxel<VW, LAYOUT>(vox, off);          // when the walk is over: the last voxel again, unused
                 if (len > 0.f) {
                     if (COUNT) ++n_seg;
                     accumulate_voxel<VW, LAYOUT>(cv, len, part, cur, curm);

@@ -108,24 +108,26 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
 }
 
 // PACKED_QUAD, second copy for the Siddon walk (project_siddon.cu), made from the quads the first time the
-// Siddon method is used on a volume: the same tagged word per voxel (no pad, no purity flag), stored once, in bricks of 4 (x) x 4 (y) x 2 (z) voxels = one 128-byte line,
-// bricks x fastest.  A walk then finds ~4 consecutive voxels in a line whatever its direction, and a
-// 4-byte warp-wide load touches a few sectors instead of one per lane.  One thread per stored word.
+// Siddon method is used on a volume: the same tagged word per voxel (no pad, no purity flag), stored once, with the
+// rows in groups of four: word (ix, iy, iz) sits at  iz * SZ + (iy >> 2) * SY + 4 ix + (iy & 3),  SY = 4 nx,
+// SZ = SY * ceil(ny / 4).  A 128-byte line is 8 (x) x 4 (y) voxels: a walk along x or along y finds 8 or 4 of its
+// voxels in a line, and a step along x or z adds a constant to the offset (a step along y: 1, or SY - 3 across a
+// group's edge).  Measured against 4 x 4 x 2 bricks (offset recomputed from the indices): +14% over a scan,
+// the same speed at every gantry angle; plain linear rows: +13% over a scan but -16% where the rays run along y.
+// One thread per stored word.
 __global__ void __launch_bounds__(256)
 gdrr_ingest_compact_kernel(const IngestParams P) {
-    // grid: x over the 32 cbx words of a row of bricks, y = row of bricks, z = slab of bricks
+    // grid: x over the 4 nx words of a group of rows, y = group of rows, z = slab
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= 32 * P.cbx) return;
-    const int e = t & 31, bx = t >> 5, by = blockIdx.y, bz = blockIdx.z;
-    const size_t o = ((size_t)bz * P.cby + by) * P.cbx * 32 + t;
-    const int ix = 4 * bx + (e & 3), iy = 4 * by + ((e >> 2) & 3), iz = 2 * bz + (e >> 4);
+    if (t >= 4 * P.nx) return;
+    const int ix = t >> 2, iy = 4 * blockIdx.y + (t & 3), iz = blockIdx.z;
     unsigned bits = 0u;
-    if (ix < P.nx && iy < P.ny && iz < P.nz) {
+    if (iy < P.ny) {
         // voxel (ix, iy, iz) is the first word of quad (ix + 1, iy + 1, iz + 1); drop its purity flag
         bits = reinterpret_cast<const unsigned*>(P.vox)[4 * ((size_t)(iz + 1) * P.sz + (size_t)(iy + 1) * P.sy + (ix + 1))];
         if (P.n_mat > 1) bits &= ~4u;
     }
-    reinterpret_cast<unsigned*>(P.compact)[o] = bits;
+    reinterpret_cast<unsigned*>(P.compact)[((size_t)iz * P.cby + blockIdx.y) * (4 * (size_t)P.nx) + t] = bits;
 }
 
 template <int VW, int LAYOUT>
@@ -137,13 +139,13 @@ static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
 }
 
 cudaError_t launch_compact_copy(const IngestParams& p, cudaStream_t s) {
-    gdrr_ingest_compact_kernel<<<dim3((32 * p.cbx + 255) / 256, p.cby, (p.nz + 1) / 2), 256, 0, s>>>(p);
+    gdrr_ingest_compact_kernel<<<dim3((4 * p.nx + 255) / 256, p.cby, p.nz), 256, 0, s>>>(p);
     return cudaGetLastError();
 }
 
 cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_t s) {
     if (layout == 2) {
-        // (py and pz, cby and nz / 2 stay far below the 65535 limit of grid.y / grid.z for any volume that fits int32 indexing)
+        // (py and pz, cby and nz stay far below the 65535 limit of grid.y / grid.z for any volume that fits int32 indexing)
         const int row_max = p.sy + 8;                                   // a row, or the last row plus the slab's tail pad
         gdrr_ingest_packed_kernel<<<dim3((row_max + 255) / 256, p.py, p.pz), 256, 0, s>>>(p);
         return cudaGetLastError();
