@@ -336,7 +336,7 @@ def run_b200(args):
     # C3 per launch; per-projection figure x the projections of one launch here); other workloads: not captured
     NCU_DRAM_PER_PROJECTION = {("C3", "gdrr_project_staged_kernel"): (3.390962e9 + 11.264e6) / 8,      # profiles/r01_staged_kernel_ncu.md
                                ("C3", "gdrr_project_packed_kernel"): (3.194201e9 + 10.405888e6) / 8,    # profiles/r01_packed_kernel_ncu.md
-                               ("C3", "gdrr_project_siddon_kernel"): (656.83712e6 + 10.174976e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
+                               ("C3", "gdrr_project_siddon_kernel"): (671.44704e6 + 9.620992e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
     if ncu_traffic is None and (args.workload, kname.split(" ")[0]) in NCU_DRAM_PER_PROJECTION:
         ncu_traffic = NCU_DRAM_PER_PROJECTION[(args.workload, kname.split(" ")[0])] * launch_proj
@@ -350,11 +350,11 @@ def run_b200(args):
                 "ncu_identified_bound": {
                     "gdrr_project_staged_kernel": "instruction issue: 74.6% of issue slots, L1 data pipe 60% (profiles/r01_staged_kernel_ncu.md)",
                     "gdrr_project_packed_kernel": "L1 data-pipe wavefronts: 72% over a scan, 85-89% on one angle (profiles/r01_packed_kernel_ncu.md)",
-                    "gdrr_project_siddon_kernel": "instruction issue: 78% of issue slots, L1 13% (profiles/r01_siddon_kernel_ncu.md)",
+                    "gdrr_project_siddon_kernel": "instruction issue: 71% of issue slots, L1 20%; largest stall the wait for the next voxel (profiles/r01_siddon_kernel_ncu.md)",
                 }.get(kname.split(" ")[0], "not profiled"),
                 # busy fraction of that bound in the committed `ncu --set full` capture (8 projections of C3), not re-measured here
                 "ncu_bound_busy_frac": {"gdrr_project_staged_kernel": 0.746, "gdrr_project_packed_kernel": 0.715,
-                                        "gdrr_project_siddon_kernel": 0.781}.get(kname.split(" ")[0]),
+                                        "gdrr_project_siddon_kernel": 0.709}.get(kname.split(" ")[0]),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
                         "algorithmic": "device-layout volume once per projection + 4 B per pixel"}}
