@@ -7,13 +7,13 @@
 // next to a tile edge that is not an image edge go stale one ring per sweep, and after t sweeps
 // the cells at least t away from such edges are exact; those include the CTA's output tile.
 // At an image edge the tile ends with the image and clamping the neighbour index to the tile IS
-// the replicated edge.  fp32 arithmetic (IEEE division).
+// the replicated edge.  fp32 arithmetic; S_hat / S by reciprocal and multiply (2 ulp, far inside the tolerance).
 #include "gdrr_internal.h"
 
 namespace gdrr {
 
-constexpr int kDnTileW = 64, kDnTileH = 16, kSweeps = 4;
-constexpr int kDnW = kDnTileW + 2 * kSweeps, kDnH = kDnTileH + 2 * kSweeps;     // 72 x 24 cells
+constexpr int kDnTileW = 128, kDnTileH = 32, kSweeps = 4;
+constexpr int kDnW = kDnTileW + 2 * kSweeps, kDnH = kDnTileH + 2 * kSweeps;     // 136 x 40 cells
 
 struct DenoiseParams {
     const float* s_hat;     // [n_images][nv][nu]
@@ -60,7 +60,7 @@ gdrr_denoise_kernel(const DenoiseParams P) {
             if (col && ly < h) {
                 const float s = cur[ly][lx];
                 const float sum = cur[ly][lxp] + cur[min(ly + 1, h - 1)][lx] + cur[ly][lxm] + cur[max(ly - 1, 0)][lx];
-                const float v = P.one_minus_w * s + P.w4 * (sum - P.inv_beta * (1.f - hat[r] / s));
+                const float v = P.one_minus_w * s + P.w4 * (sum - P.inv_beta * (1.f - __fdividef(hat[r], s)));
                 nxt[ly][lx] = fmaxf(v, P.floor_value);
             }
         }
