@@ -286,9 +286,9 @@ cudaError_t ensure_compact(const gdrr_volume* vol, cudaStream_t s) {
 
 // Does staging pay?  Extent, in voxels per axis, of the beam of a 16 x 16-pixel CTA over 16 steps at the
 // depth of the box centre, averaged over the requested projections, against the 14 x 14 x 11-quad box (a chunk
-// whose beam does not fit is gathered anyway, after paying for its bounding box).  Thresholds measured on C3:
-// circle and helix (mean extents 10.5, 10.5, 6.6) +15%; orbit tilted 20 degrees (10.5, 12.7, 9.0) +4%;
-// tilted 35 degrees (10.5, 13.4, 10.1) -15%.
+// whose beam does not fit is gathered anyway, after paying for its bounding box).  Thresholds measured on C3
+// (staged against gather): circle and helix (mean extents 10.5, 10.5, 6.6) +19%; orbit tilted 10 degrees
+// (10.5, 11.8, 8.0) +22%; tilted 20 degrees (10.5, 12.7, 9.0) -2%; tilted 35 degrees (10.5, 13.4, 10.1) -20%.
 bool beam_fits(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& g) {
     double ext[3] = {0.0, 0.0, 0.0};
     for (int p = g.proj_begin; p < g.proj_begin + g.proj_count; ++p) {
@@ -309,7 +309,7 @@ bool beam_fits(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& 
                        16.0 * g.step * std::fabs(P[a] - S[a]) / std::sqrt(sp)) / vol->d[a];
     }
     for (int a = 0; a < 3; ++a) ext[a] /= (double)g.proj_count;
-    return ext[0] <= 12.9 && ext[1] <= 12.9 && ext[2] <= 9.1;
+    return ext[0] <= 12.5 && ext[1] <= 12.5 && ext[2] <= 8.9;
 }
 
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {

@@ -185,4 +185,38 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
     }
 }
 
+// The unpredicated chunk in PAIRS (as the staged sampler's pair loop): both cells of two consecutive samples are
+// requested, one vote decides for the pair, the fractions come from packed subtractions.
+template <int VW>
+__device__ __forceinline__ void run_chunk_pairs(const Sampler& S, const ChunkBase& b, int cnt, RayAcc<VW>& A) {
+    int qx = b.qx, qy = b.qy, qz = b.qz;
+    const int idx0 = elem_index(b.cx, b.cy, b.cz, S.sy, S.sz);
+#pragma unroll 2
+    for (int s = 0; s < cnt; s += 2) {
+        const int i0 = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
+        const unsigned bx0 = frac_bits(qx, S.fmask, S.fone), by0 = frac_bits(qy, S.fmask, S.fone),
+                       bz0 = frac_bits(qz, S.fmask, S.fone);
+        qx += S.dqx; qy += S.dqy; qz += S.dqz;
+        const int i1 = sample_index(idx0, qx, qy, qz, S.sy, S.sz);
+        const uint4 a0 = __ldg(S.vol0 + i0), c0 = __ldg(S.vol1 + i0);
+        const uint4 a1 = __ldg(S.vol0 + i1), c1 = __ldg(S.vol1 + i1);
+        const unsigned bx1 = frac_bits(qx, S.fmask, S.fone), by1 = frac_bits(qy, S.fmask, S.fone),
+                       bz1 = frac_bits(qz, S.fmask, S.fone);
+        qx += S.dqx; qy += S.dqy; qz += S.dqz;
+        float fx0, fx1, fy0, fy1, fz0, fz1;
+        sub_one2(bx0, bx1, fx0, fx1);
+        sub_one2(by0, by1, fy0, fy1);
+        sub_one2(bz0, bz1, fz0, fz1);
+        bool fast = true;
+        if (VW > 1) fast = __all_sync(0xffffffffu, ((((a0.x ^ A.curm4) | (a1.x ^ A.curm4)) & 7u) == 0u));
+        if (fast) {
+            A.cur += blend_cell(a0, c0, fx0, fy0, fz0);
+            A.cur += blend_cell(a1, c1, fx1, fy1, fz1);
+        } else {
+            blend_sample<VW, false>(a0, c0, fx0, fy0, fz0, A.cur, A.curm4, A.part);
+            blend_sample<VW, false>(a1, c1, fx1, fy1, fz1, A.cur, A.curm4, A.part);
+        }
+    }
+}
+
 }  // namespace gdrr

@@ -110,7 +110,7 @@ gdrr_project_packed_kernel(const ProjectParams P) {
 
         const bool mine = rel < un && rel + (unsigned)cnt <= un;         // this lane owns the whole chunk
         if (__all_sync(0xffffffffu, mine) && !(cnt & 1))
-            run_chunk<VW, false>(S, b, cnt, rel, un, A);
+            run_chunk_pairs<VW>(S, b, cnt, A);
         else
             run_chunk<VW, true>(S, b, cnt, rel, un, A);
 
