@@ -37,7 +37,8 @@ struct gdrr_context {
     float* bt_dev = nullptr;
     float* flu_dev = nullptr;
     // misc
-    int* flag_dev = nullptr;
+    int* flag_host = nullptr;       // pinned, mapped: the ingest kernel sets it through flag_dev if it meets a bad material
+    int* flag_dev = nullptr;        //   (device address of flag_host)
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
@@ -351,8 +352,13 @@ int gdrr_create_context(int cuda_device, gdrr_context** out) {
     ctx->device = cuda_device;
     DeviceGuard guard(cuda_device);
     if (guard.status != cudaSuccess) { delete ctx; return cuda_fail(nullptr, guard.status, "cudaSetDevice"); }
-    e = cudaMalloc(&ctx->flag_dev, sizeof(int));
-    if (e != cudaSuccess) { delete ctx; return cuda_fail(nullptr, e, "cudaMalloc(flag)"); }
+    e = cudaHostAlloc(&ctx->flag_host, sizeof(int), cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->flag_dev, ctx->flag_host, 0);
+    if (e != cudaSuccess) {
+        if (ctx->flag_host) cudaFreeHost(ctx->flag_host);
+        delete ctx;
+        return cuda_fail(nullptr, e, "cudaHostAlloc(flag)");
+    }
     *out = ctx;
     return GDRR_OK;
 }
@@ -361,7 +367,8 @@ int gdrr_destroy_context(gdrr_context* ctx) {
     if (!ctx) return GDRR_OK;
     DeviceGuard guard(ctx->device);
     free_dev(ctx->poses_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
-    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->flag_dev);
+    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev);
+    if (ctx->flag_host) { cudaFreeHost(ctx->flag_host); ctx->flag_host = nullptr; ctx->flag_dev = nullptr; }
     for (int k = 0; k < 2; ++k) {
         if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
         if (ctx->ev_free[k]) cudaEventDestroy(ctx->ev_free[k]);
@@ -413,8 +420,8 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    cudaError_t e = cudaMemsetAsync(ctx->flag_dev, 0, sizeof(int), s);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(flag)");
+    *ctx->flag_host = 0;            // (no kernel of this context is writing it: every ingest is waited for below)
+    cudaError_t e = cudaSuccess;
     IngestParams ip;
     ip.rho = rho_dev; ip.mat = material_dev; ip.vox = workspace_dev;
     ip.nx = nx; ip.ny = ny; ip.nz = nz;
@@ -430,10 +437,9 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     e = launch_ingest(ip, vw, layout, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel launch");
     ctx->launches += 1;
-    int bad = 0;
-    e = cudaMemcpyAsync(&bad, ctx->flag_dev, sizeof(int), cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel");
+    const int bad = *(volatile int*)ctx->flag_host;
     if (bad) return fail(ctx, GDRR_ERR_INVALID_ARG, "a material index is >= n_materials (%d)", n_materials);
 
     gdrr_volume* v = new (std::nothrow) gdrr_volume;
