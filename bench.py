@@ -334,7 +334,7 @@ def run_b200(args):
     hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
     # dram__bytes_read + dram__bytes_write per launch, from the committed `ncu --set full` captures (8 projections of
     # C3 per launch; per-projection figure x the projections of one launch here); other workloads: not captured
-    NCU_DRAM_PER_PROJECTION = {("C3", "gdrr_project_staged_kernel"): (3.390962e9 + 11.264e6) / 8,      # profiles/r01_staged_kernel_ncu.md
+    NCU_DRAM_PER_PROJECTION = {("C3", "gdrr_project_staged_kernel"): (3.392791e9 + 9.7344e6) / 8,      # profiles/r01_staged_kernel_ncu.md
                                ("C3", "gdrr_project_packed_kernel"): (3.194201e9 + 10.405888e6) / 8,    # profiles/r01_packed_kernel_ncu.md
                                ("C3", "gdrr_project_siddon_kernel"): (671.44704e6 + 9.620992e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
     ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
@@ -348,12 +348,12 @@ def run_b200(args):
                                f"{'segment' if args.method == 'siddon' else 'sample'} through L1",
                 "samples_per_clk_per_sm": n_samples / (kernel_ms * 1e-3) / (SM_COUNT * peaks["sm_max_mhz"] * 1e6),
                 "ncu_identified_bound": {
-                    "gdrr_project_staged_kernel": "instruction issue: 74.6% of issue slots, L1 data pipe 60% (profiles/r01_staged_kernel_ncu.md)",
+                    "gdrr_project_staged_kernel": "instruction issue: 77.6% of issue slots, L1 data pipe 63% (profiles/r01_staged_kernel_ncu.md)",
                     "gdrr_project_packed_kernel": "L1 data-pipe wavefronts: 72% over a scan, 85-89% on one angle (profiles/r01_packed_kernel_ncu.md)",
                     "gdrr_project_siddon_kernel": "instruction issue: 71% of issue slots, L1 20%; largest stall the wait for the next voxel (profiles/r01_siddon_kernel_ncu.md)",
                 }.get(kname.split(" ")[0], "not profiled"),
                 # busy fraction of that bound in the committed `ncu --set full` capture (8 projections of C3), not re-measured here
-                "ncu_bound_busy_frac": {"gdrr_project_staged_kernel": 0.746, "gdrr_project_packed_kernel": 0.715,
+                "ncu_bound_busy_frac": {"gdrr_project_staged_kernel": 0.776, "gdrr_project_packed_kernel": 0.715,
                                         "gdrr_project_siddon_kernel": 0.709}.get(kname.split(" ")[0]),
                 "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],

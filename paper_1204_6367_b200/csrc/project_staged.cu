@@ -13,7 +13,10 @@
 // interval index k and a chunk of kStageK indices is a thin curved slab of the beam.  Per
 // chunk every thread contributes the cells of its first and last sample of the chunk (the
 // cells in between are bracketed by them: positions are linear in k) to a CTA-wide bounding
-// box; thread 0 issues the copy of that box for chunk c + 1 while chunk c is sampled.  The box
+// box (one redux per warp, its lane 0 posts it with shared atomics and counts the warp in); the
+// warp that posts LAST requests the box for chunk c + 1 while chunk c is sampled -- no CTA barrier in
+// the loop: a warp that has posted has finished chunk c - 1, whose stage the new box overwrites, and
+// goes on to chunk c; it waits only for its own chunk's box (mbarrier).  The box
 // has a fixed shape (kBX x kBY x kBZ quads: a tensor map fixes its box); a chunk whose
 // bounding box does not fit (other geometries) is sampled from global memory by the gather
 // path's own routine, so the result never depends on the staging.
@@ -49,6 +52,9 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
 }
 // box of the 3-D tensor (words along x, rows, slabs) at (c0, c1, c2) -> shared memory, completes on `bar`
 __device__ __forceinline__ void tma_load_box(void* dst, const CUtensorMap* map, int c0, int c1, int c2,
@@ -146,6 +152,7 @@ struct StageCtl {
     int lin[2];                    // stage s: element of cell (cx, cy, cz) = lin + (cz kBY + cy) kBX + cx
     int fit[2];                    // stage s holds the box of its chunk (else: gather from global memory)
     int krange[2];                 // smallest first / largest last+1 interval index of the CTA's rays
+    int arrived[3];                // warps that have put their share into bb[slot]
 };
 
 template <int VW>
@@ -165,6 +172,7 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             for (int a = 0; a < 3; ++a) { ctl.bb[m][a] = 0x7fffffff; ctl.bb[m][3 + a] = (int)0x80000000; }
         ctl.krange[0] = 0x7fffffff;
         ctl.krange[1] = (int)0x80000000;
+        ctl.arrived[0] = ctl.arrived[1] = ctl.arrived[2] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -260,40 +268,55 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
                     mx[a] = max(c_lo, c_hi);
                 }
             }
-            // every lane calls the atomics with its own values (neutral ones if it has no sample in the chunk):
-            // the compiler aggregates a warp-uniform shared atomic into one redux + one atomic by an elected lane
+            // the warp's share, posted by lane 0; the warp that arrives last (its lane 0) gets `true`
+            bool last = false;
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                atomicMin(&ctl.bb[slot][a], mn[a]);
-                atomicMax(&ctl.bb[slot][3 + a], mx[a]);
+                mn[a] = __reduce_min_sync(0xffffffffu, mn[a]);
+                mx[a] = __reduce_max_sync(0xffffffffu, mx[a]);
             }
+            if (lane == 0) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    atomicMin(&ctl.bb[slot][a], mn[a]);
+                    atomicMax(&ctl.bb[slot][3 + a], mx[a]);
+                }
+                __threadfence_block();
+                last = atomicAdd(&ctl.arrived[slot], 1) == kThreads / 32 - 1;
+                if (last) __threadfence_block();
+            }
+            return last;
         };
         // thread 0: request the box of chunk m into stage m & 1 if it fits
         auto issue = [&](int m, int slot) {
-            const int* bb = ctl.bb[slot];
+            int* bb = ctl.bb[slot];
             const int st = m & 1;
-            const bool fit = bb[0] <= bb[3] && bb[3] - bb[0] + 1 <= kBX && bb[4] - bb[1] + 1 <= kBY &&
-                             bb[5] - bb[2] + 2 <= kBZ;
+            const int b0 = bb[0], b1 = bb[1], b2 = bb[2];
+            const bool fit = b0 <= bb[3] && bb[3] - b0 + 1 <= kBX && bb[4] - b1 + 1 <= kBY && bb[5] - b2 + 2 <= kBZ;
+            // the slot is free for the chunk three ahead (no warp reaches that one before the box requested here
+            // and the next one have been waited for)
+            for (int a = 0; a < 3; ++a) { bb[a] = 0x7fffffff; bb[3 + a] = (int)0x80000000; }
+            ctl.arrived[slot] = 0;
             ctl.fit[st] = fit;
             // element of cell (cx, cy, cz) in the stage: lin + (cz kBY + cy) kBX + cx
-            ctl.lin[st] = st * kStageElems - ((bb[2] * kBY + bb[1]) * kBX + bb[0]);
+            ctl.lin[st] = st * kStageElems - ((b2 * kBY + b1) * kBX + b0);
+            // the phase of bar[st] completes either way and orders fit / lin before their readers
             if (fit) {
                 mbar_arrive_expect_tx(&ctl.bar[st], kBoxBytes);
-                tma_load_box(s_box + st * kStageElems, &tmap, 4 * bb[0], bb[1], bb[2], &ctl.bar[st]);
+                tma_load_box(s_box + st * kStageElems, &tmap, 4 * b0, b1, b2, &ctl.bar[st]);
+            } else {
+                mbar_arrive(&ctl.bar[st]);
             }
         };
 
-        contribute(c_begin * kStageK, 0);
-        __syncthreads();
-        if (threadIdx.x == 0) issue(0, 0);
+        // No CTA barrier in the loop: a warp posts its share of the next chunk's box (it has then finished the
+        // chunk before, whose stage the new box overwrites) and goes on; whichever warp posts last requests the box.
+        if (contribute(c_begin * kStageK, 0)) issue(0, 0);
         unsigned phases = 0u;                    // bit st: parity of the next completion of bar[st]
-        int slot1 = 1, slot2 = 2;                // bounding-box slots of chunks m + 1 and m + 2 (m % 3 rotation)
+        int slot1 = 1;                           // bounding-box slot of chunk m + 1 (m % 3 rotation)
 
         for (int m = 0; m < nchunks; ++m) {
             const int st = m & 1;
-            if (threadIdx.x == 0) {              // the slot chunk m + 2 will use: consumed two iterations ago
-                for (int a = 0; a < 3; ++a) { ctl.bb[slot2][a] = 0x7fffffff; ctl.bb[slot2][3 + a] = (int)0x80000000; }
-            }
             // chunk m: working copy of its base; then the base moves on to chunk m + 1
             const int kc = (c_begin + m) * kStageK;
             const int wqx = qb[0] >> (kBaseBits - kFracBits), wqy = qb[1] >> (kBaseBits - kFracBits),
@@ -308,15 +331,9 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
                     cb[a] += dc[a];
                     qb[a] = q & ((1 << kBaseBits) - 1);
                 }
-                contribute(kc + kStageK, slot1);
+                if (contribute(kc + kStageK, slot1)) issue(m + 1, slot1);
             }
-            __syncthreads();                     // box of m + 1 known; everyone is done with stage st ^ 1
-            if (threadIdx.x == 0 && m + 1 < nchunks) issue(m + 1, slot1);
-            {
-                const int s0 = 3 - slot1 - slot2;    // rotate (slot of m, slot1, slot2) -> (slot1, slot2, slot of m)
-                slot1 = slot2;
-                slot2 = s0;
-            }
+            slot1 = slot1 == 2 ? 0 : slot1 + 1;
 
             const unsigned rel = (unsigned)(kc - j0);
             const bool mine = rel < un && rel + (unsigned)kStageK <= un;     // this lane owns the whole chunk
@@ -324,9 +341,9 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
 #pragma unroll
             for (int k = 0; k < VW; ++k) A.part[k] = 0.f;
 
+            mbar_wait(&ctl.bar[st], (phases >> st) & 1u);      // box landed (or: chunk does not fit); fit / lin valid
+            phases ^= 1u << st;
             if (ctl.fit[st]) {
-                mbar_wait(&ctl.bar[st], (phases >> st) & 1u);
-                phases ^= 1u << st;
                 const int idx0 = rel_cell + ctl.lin[st];
                 if (all_mine) run_chunk_staged_pairs<VW>(S, wqx, wqy, wqz, idx0, A);
                 else run_chunk_staged<VW, true>(S, wqx, wqy, wqz, idx0, kStageK, rel, un, A);
