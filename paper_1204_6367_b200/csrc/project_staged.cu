@@ -276,14 +276,16 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
                 mx[a] = __reduce_max_sync(0xffffffffu, mx[a]);
             }
             if (lane == 0) {
+                // (PTX reductions: the compiler would wrap atomicMin / atomicMax in a second warp reduction; the
+                // acq_rel counter orders the six before it and, in the warp that arrives last, the others' before its reads)
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
-                    atomicMin(&ctl.bb[slot][a], mn[a]);
-                    atomicMax(&ctl.bb[slot][3 + a], mx[a]);
+                    asm volatile("red.relaxed.cta.shared::cta.min.s32 [%0], %1;" ::"r"(smem_addr(&ctl.bb[slot][a])), "r"(mn[a]) : "memory");
+                    asm volatile("red.relaxed.cta.shared::cta.max.s32 [%0], %1;" ::"r"(smem_addr(&ctl.bb[slot][3 + a])), "r"(mx[a]) : "memory");
                 }
-                __threadfence_block();
-                last = atomicAdd(&ctl.arrived[slot], 1) == kThreads / 32 - 1;
-                if (last) __threadfence_block();
+                unsigned before;
+                asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(before) : "r"(smem_addr(&ctl.arrived[slot])) : "memory");
+                last = before == (unsigned)(kThreads / 32 - 1);
             }
             return last;
         };
