@@ -115,6 +115,26 @@ def test_pose_paths_siddon(gdrr, workloads_cache):
         check_ray_table(tab.cpu().numpy(), ref["ray_table"])
 
 
+def test_pose_edge_cases(gdrr):
+    """A pose looking away from the volume: flat field, n = 0 everywhere; a source inside the volume box: error."""
+    rho = np.ones((8, 8, 8), dtype=np.float32)
+    w = tiny_workload(rho, spacing=(2.0, 2.0, 2.0), nu=20, nv=18, du=4.0, dv=4.0, sad=300.0, sdd=500.0)
+    away = trajectories.circular_poses(300.0, 500.0, 0.0, [0.0, 1.0])
+    away[:, 3:6] = 2.6 * away[:, 0:3]                       # detector behind the source
+    ref = oracle.project(w.with_poses(away))
+    for layout in (0, 1, 2):
+        with gdrr.Projector(w.with_poses(away), layout=layout) as pr:
+            sig, li, tab = pr.project(want_li=True, want_table=True)
+            check_ray_table(tab.cpu().numpy(), ref["ray_table"])
+            assert torch.count_nonzero(li).item() == 0
+            check_signal(sig.cpu().numpy(), ref["signal"], "away")
+    inside = trajectories.circular_poses(300.0, 500.0, 0.0, [0.0])
+    inside[0, 0:3] = (1.0, -2.0, 0.5)
+    with gdrr.Projector(w.with_poses(inside)) as pr:
+        with pytest.raises(gdrr.GdrrError):
+            pr.project()
+
+
 def test_pose_argument_errors(gdrr):
     ctx = gdrr.gdrr_create_context(0)
     try:

@@ -194,3 +194,29 @@ def test_pose_ray_geometry_matches_a_direct_construction():
     assert np.allclose(r["S"], pose[0:3])
     assert r["L"] == pytest.approx(np.linalg.norm(d), rel=1e-14)
     assert np.allclose(r["dir"], d / np.linalg.norm(d), atol=1e-14)
+
+
+def test_trajectory_generators_give_orthonormal_frames_at_the_stated_distances():
+    phis = np.radians([0.0, 33.0, 180.0, 311.0])
+    for poses in (trajectories.circular_poses(1000.0, 1500.0, 0.0, phis),
+                  trajectories.helical_poses(1000.0, 1500.0, phis, 40.0, z0_mm=-5.0),
+                  trajectories.c_arm_poses(1000.0, 1500.0, phis, 0.4),
+                  trajectories.free_poses(4, 1000.0, 1500.0, seed=1)):
+        S, P, uh, vh = poses[:, 0:3], poses[:, 3:6], poses[:, 6:9], poses[:, 9:12]
+        assert np.allclose(np.linalg.norm(uh, axis=1), 1.0, atol=1e-12)
+        assert np.allclose(np.linalg.norm(vh, axis=1), 1.0, atol=1e-12)
+        assert np.allclose(np.sum(uh * vh, axis=1), 0.0, atol=1e-12)
+        nrm = np.cross(uh, vh)
+        # source-to-detector distance along the detector normal is SDD
+        assert np.allclose(np.abs(np.sum((P - S) * nrm, axis=1)), 1500.0, rtol=1e-12)
+
+
+def test_pose_that_looks_away_from_the_volume_gives_the_flat_field():
+    rho = np.ones((8, 8, 8), dtype=np.float32)
+    w = tiny_workload(rho, spacing=(2.0, 2.0, 2.0), nu=6, nv=5, du=4.0, dv=4.0, sad=300.0, sdd=500.0)
+    pose = trajectories.circular_poses(300.0, 500.0, 0.0, [0.0])
+    pose[0, 3] = -800.0                      # detector behind the source: every ray leaves the volume behind
+    out = oracle.project(w.with_poses(pose))
+    assert np.all(out["ray_table"][..., 1] == 0)
+    assert np.all(out["line_integrals"] == 0.0)
+    assert np.allclose(out["signal"], 1.0, rtol=1e-15)
