@@ -184,6 +184,7 @@ int fill_geom(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int pro
         g.hi[a] = vol->c[a] + half;
         g.c[a] = vol->c[a];
         g.d[a] = vol->d[a];
+        g.inv_d[a] = 1.0 / vol->d[a];
         g.ofs[a] = 0.5 * (double)(n[a] - 1) + 1.0;
         if (vol->d[a] < dmin) dmin = vol->d[a];
     }

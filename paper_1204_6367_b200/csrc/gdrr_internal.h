@@ -32,6 +32,7 @@ struct GeomParams {
     double step;                    // dl
     double lo[3], hi[3];            // volume box
     double c[3], d[3];              // box centre, voxel size
+    double inv_d[3];                // 1 / d (host): the index-space line is formed with multiplications
     double ofs[3];                  // 0.5 * (N - 1) + 1: world -> padded index coordinates
     const double* poses;            // [n_proj][12] source S, detector origin P, u_hat, v_hat; device
     int nu, nv;
