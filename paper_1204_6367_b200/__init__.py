@@ -142,8 +142,21 @@ def gdrr_version():
     return _lib.gdrr_version().decode()
 
 
+class _Context(ctypes.c_void_p):
+    """The gdrr_context* handle.  The C ABI cannot see the sizes of the caller's device buffers, so the binding
+    remembers the detector shape and the material count it passed in and checks every output tensor against them."""
+    nu = nv = n_mat = None
+
+
+def _plane(ctx, proj_count, per_pixel=1, what="gdrr_set_geometry"):
+    """Elements an output of `proj_count` projections needs (0 if the shape is not known on this side)."""
+    if not isinstance(ctx, _Context) or ctx.nu is None:
+        return 0
+    return int(proj_count) * ctx.nu * ctx.nv * per_pixel
+
+
 def gdrr_create_context(cuda_device=0):
-    out = ctypes.c_void_p()
+    out = _Context()
     _check(_lib.gdrr_create_context(int(cuda_device), ctypes.byref(out)))
     return out
 
@@ -223,6 +236,8 @@ def gdrr_set_geometry(ctx, sad_mm, sdd_mm, theta_rad, nu, nv, du_mm, dv_mm, u_of
     _check(_lib.gdrr_set_geometry(ctx, float(sad_mm), float(sdd_mm), float(theta_rad), int(nu),
                                   int(nv), float(du_mm), float(dv_mm), float(u_offset_mm),
                                   float(v_offset_mm), int(phi.shape[0]), phi_p, float(step_mm)), ctx)
+    if isinstance(ctx, _Context):
+        ctx.nu, ctx.nv = int(nu), int(nv)
 
 
 def gdrr_set_geometry_poses(ctx, nu, nv, du_mm, dv_mm, u_offset_mm, v_offset_mm, poses, step_mm):
@@ -230,6 +245,8 @@ def gdrr_set_geometry_poses(ctx, nu, nv, du_mm, dv_mm, u_offset_mm, v_offset_mm,
     ps, ps_p = _host(np.ascontiguousarray(poses, dtype=np.float64).reshape(-1, 12), np.float64)
     _check(_lib.gdrr_set_geometry_poses(ctx, int(nu), int(nv), float(du_mm), float(dv_mm), float(u_offset_mm),
                                         float(v_offset_mm), int(ps.shape[0]), ps_p, float(step_mm)), ctx)
+    if isinstance(ctx, _Context):
+        ctx.nu, ctx.nv = int(nu), int(nv)
 
 
 def gdrr_set_spectrum(ctx, phi_weight, response, mu_hat, fluence_map=None, bowtie_mu=None,
@@ -248,28 +265,32 @@ def gdrr_set_spectrum(ctx, phi_weight, response, mu_hat, fluence_map=None, bowti
     if bm is not None and bm.shape != (n_e,):
         raise ValueError("bowtie_mu must be [n_energy]")
     _check(_lib.gdrr_set_spectrum(ctx, n_e, n_mat, pw_p, rs_p, mu_p, fl_p, bm_p, bt_p), ctx)
+    if isinstance(ctx, _Context):
+        ctx.n_mat = int(n_mat)
 
 
 def gdrr_project(ctx, vol, proj_begin, proj_count, signal_dev, line_integrals_dev=None,
                  ray_table_dev=None, stream=None):
+    n_mat = ctx.n_mat if isinstance(ctx, _Context) and ctx.n_mat else 0
     _check(_lib.gdrr_project(ctx, vol, int(proj_begin), int(proj_count),
-                             _dev(signal_dev, "float32", 0, "signal_dev"),
-                             _dev(line_integrals_dev, "float32", 0, "line_integrals_dev"),
-                             _dev(ray_table_dev, "int32", 0, "ray_table_dev"), _stream(stream)), ctx)
+                             _dev(signal_dev, "float32", _plane(ctx, proj_count), "signal_dev"),
+                             _dev(line_integrals_dev, "float32", _plane(ctx, proj_count, n_mat), "line_integrals_dev"),
+                             _dev(ray_table_dev, "int32", _plane(ctx, proj_count, 2), "ray_table_dev"),
+                             _stream(stream)), ctx)
 
 
 def gdrr_project_host(ctx, vol, proj_begin, proj_count, signal_host, signal_stage_dev, stage_proj,
                       stream=None):
     _check(_lib.gdrr_project_host(ctx, vol, int(proj_begin), int(proj_count),
-                                  _host_ptr(signal_host, "float32", 0),
-                                  _dev(signal_stage_dev, "float32", 0, "signal_stage_dev"),
+                                  _host_ptr(signal_host, "float32", _plane(ctx, proj_count)),
+                                  _dev(signal_stage_dev, "float32", _plane(ctx, stage_proj), "signal_stage_dev"),
                                   int(stage_proj), _stream(stream)), ctx)
 
 
 def gdrr_ray_setup(ctx, vol, proj_begin, proj_count, ray_table_dev=None, n_samples_dev=None,
                    stream=None):
     _check(_lib.gdrr_ray_setup(ctx, vol, int(proj_begin), int(proj_count),
-                               _dev(ray_table_dev, "int32", 0, "ray_table_dev"),
+                               _dev(ray_table_dev, "int32", _plane(ctx, proj_count, 2), "ray_table_dev"),
                                _dev(n_samples_dev, "int64", 1, "n_samples_dev"), _stream(stream)), ctx)
 
 
@@ -297,7 +318,8 @@ def gdrr_set_sampler(ctx, sampler):
 
 def gdrr_siddon_segments(ctx, vol, proj_begin, proj_count, n_segments_dev, stream=None):
     _check(_lib.gdrr_siddon_segments(ctx, vol, int(proj_begin), int(proj_count),
-                                     _dev(n_segments_dev, "int32", 0, "n_segments_dev"), _stream(stream)), ctx)
+                                     _dev(n_segments_dev, "int32", _plane(ctx, proj_count), "n_segments_dev"),
+                                     _stream(stream)), ctx)
 
 
 def gdrr_kernel_launches(ctx):
@@ -364,6 +386,8 @@ class Projector:
             self.vol = gdrr_create_volume_host(self.ctx, rho_host, mat_host, w.dims, w.spacing, w.centre,
                                                w.n_materials, self.layout, self.rho_stage,
                                                self.mat_stage, self.workspace)
+            if self.method == GDRR_METHOD_TEXTURE:
+                gdrr_volume_attach_texture(self.ctx, self.vol)
 
     def project(self, proj_begin=0, proj_count=None, want_li=False, want_table=False, signal=None):
         torch, w = self.torch, self.w

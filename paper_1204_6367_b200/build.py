@@ -45,17 +45,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = find_nvcc()
-    extra = os.environ.get("GDRR_NVCC_EXTRA", "").split()      # e.g. -D switches of a kernel experiment
-    cmd = [nvcc] + NVCC_FLAGS + extra + ["-shared", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [nvcc] + NVCC_FLAGS + ["-shared", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if verbose or res.returncode:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode:
         raise RuntimeError("nvcc failed building libgdrr_b200.so")
-    with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
-        # without the "Compile time" lines: they differ from build to build and the file is tracked
-        info = "\n".join(l for l in res.stderr.splitlines() if "Compile time" not in l)
-        f.write("$ " + " ".join(cmd) + "\n" + info + "\n")
+    # registers / spills / shared memory per kernel (ptxas -v): a build log, kept out of the tracked tree
+    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    with open(os.path.join(HERE, "build", "ptxas_info.txt"), "w") as f:
+        f.write("$ " + " ".join(cmd) + "\n" + res.stderr)
     return LIB
 
 

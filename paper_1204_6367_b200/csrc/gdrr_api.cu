@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -53,8 +54,12 @@ struct gdrr_volume {
     double d[3], c[3];
     int n_mat, vw, layout;
     int sy, sz;                 // PACKED_QUAD: element strides
-    void* compact = nullptr;    // PACKED_QUAD: bricked one-word-per-voxel copy (Siddon walk)
-    mutable bool compact_ready = false;   // ... made from the quads at the first Siddon use
+    void* compact = nullptr;    // PACKED_QUAD: one-word-per-voxel copy, rows in groups of four (Siddon walk)
+    // ... made from the quads at the first Siddon use: `compact_mu` serialises the callers, `compact_done` orders every
+    // later Siddon launch, on whatever stream, behind the copy kernel (ensure_compact)
+    std::mutex compact_mu;
+    bool compact_launched = false;
+    cudaEvent_t compact_done = nullptr;
     bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
     cudaArray_t tex_array = nullptr;     // optional texture variant (gdrr_volume_attach_texture)
     cudaTextureObject_t tex = 0;
@@ -273,17 +278,29 @@ bool make_tensor_map(gdrr_volume* v) {
     return r == CUDA_SUCCESS;
 }
 
-// Siddon on a packed volume walks the compact copy: make it (once, on the caller's stream) from the quads.
-cudaError_t ensure_compact(const gdrr_volume* vol, cudaStream_t s) {
-    if (vol->layout != GDRR_LAYOUT_PACKED_QUAD || vol->compact_ready) return cudaSuccess;
-    IngestParams ip = {};
-    ip.vox = vol->vox; ip.compact = vol->compact;
-    ip.nx = vol->nx; ip.ny = vol->ny; ip.nz = vol->nz;
-    ip.sy = vol->sy; ip.sz = vol->sz; ip.n_mat = vol->n_mat;
-    ip.cbx = (vol->nx + 3) / 4; ip.cby = (vol->ny + 3) / 4;
-    cudaError_t e = launch_compact_copy(ip, s);
-    if (e == cudaSuccess) { vol->compact_ready = true; vol->ctx->launches += 1; }
-    return e;
+// Siddon on a packed volume walks the compact copy.  The first caller makes it from the quads on its own stream and
+// records `compact_done` behind the copy kernel; every caller (this one included) then makes its stream wait for that
+// event, so a Siddon launch on another stream, or from another thread, can never read the copy before it is filled.
+cudaError_t ensure_compact(const gdrr_volume* cvol, cudaStream_t s) {
+    if (cvol->layout != GDRR_LAYOUT_PACKED_QUAD) return cudaSuccess;
+    gdrr_volume* vol = const_cast<gdrr_volume*>(cvol);       // the copy is a cache behind the handle, guarded by its mutex
+    std::lock_guard<std::mutex> lock(vol->compact_mu);
+    cudaError_t e = cudaSuccess;
+    if (!vol->compact_launched) {
+        if (!vol->compact_done) e = cudaEventCreateWithFlags(&vol->compact_done, cudaEventDisableTiming);
+        if (e != cudaSuccess) return e;
+        IngestParams ip = {};
+        ip.vox = vol->vox; ip.compact = vol->compact;
+        ip.nx = vol->nx; ip.ny = vol->ny; ip.nz = vol->nz;
+        ip.sy = vol->sy; ip.sz = vol->sz; ip.n_mat = vol->n_mat;
+        ip.cbx = (vol->nx + 3) / 4; ip.cby = (vol->ny + 3) / 4;
+        e = launch_compact_copy(ip, s);
+        if (e == cudaSuccess) e = cudaEventRecord(vol->compact_done, s);
+        if (e != cudaSuccess) return e;
+        vol->compact_launched = true;
+        vol->ctx->launches += 1;
+    }
+    return cudaStreamWaitEvent(s, vol->compact_done, 0);
 }
 
 // Does staging pay?  Extent, in voxels per axis, of the beam of a 16 x 16-pixel CTA over 16 steps at the
@@ -482,10 +499,11 @@ int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host, const uint
 }
 
 int gdrr_destroy_volume(gdrr_volume* vol) {
-    if (vol && (vol->tex || vol->tex_array)) {
+    if (vol && (vol->tex || vol->tex_array || vol->compact_done)) {
         DeviceGuard guard(vol->ctx->device);
         if (vol->tex) cudaDestroyTextureObject(vol->tex);
         if (vol->tex_array) cudaFreeArray(vol->tex_array);
+        if (vol->compact_done) cudaEventDestroy(vol->compact_done);
     }
     delete vol;
     return GDRR_OK;

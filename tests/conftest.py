@@ -8,6 +8,12 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+def pytest_addoption(parser):
+    parser.addoption("--full-scan", action="store_true", default=False,
+                     help="tests/test_gpu_full_scan.py: compare ALL projections of C3 and C4 with the oracle "
+                          "(about 25 minutes of oracle time) and write gpurun_out/full_parity_*.json")
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
