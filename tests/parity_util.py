@@ -19,7 +19,27 @@ def check_signal(sig_gpu, sig_ref, what=""):
     return worst
 
 
-def check_line_integrals(li_gpu, li_ref, what=""):
+FACE_TIE = 2.0 ** -12       # DESIGN.md reading Q9: a sample this close to a cell face may fall in either cell
+
+
+def face_tie_checker(w, projections):
+    """near_face(index) for check_line_integrals on full images [P][M][nv][nu] of the circular-gantry workload `w`
+    (P = len(projections), indices into w.phis): True iff the oracle's own fp64 positions of that ray have a sample
+    within FACE_TIE of a cell face (reading Q9: the fp32 path may then take the neighbouring cell, whose other
+    corners get a weight <= FACE_TIE)."""
+    import oracle
+
+    def near_face(index):
+        p, _, j, i = (int(x) for x in index)
+        gi, _ = oracle.ray_samples(w, float(w.phis[projections[p]]), i, j)
+        if not len(gi):
+            return False
+        fr = gi - np.floor(gi)
+        return bool(np.minimum(fr, 1.0 - fr).min() < FACE_TIE)
+    return near_face
+
+
+def check_line_integrals(li_gpu, li_ref, what="", near_face=None):
     li_gpu = np.asarray(li_gpu, dtype=np.float64)
     li_ref = np.asarray(li_ref, dtype=np.float64)
     assert li_gpu.shape == li_ref.shape, (li_gpu.shape, li_ref.shape)
@@ -29,8 +49,17 @@ def check_line_integrals(li_gpu, li_ref, what=""):
     bad = err > tol
     assert not bad.any(), (f"{what}: {int(bad.sum())} line integrals out of tolerance, worst "
                            f"|err| {float(err.max()):.3e} (scale {scale:.3e})")
-    # rays that miss (or cross only empty voxels) must be exactly zero
-    assert np.all(li_gpu[li_ref == 0.0] == 0.0), f"{what}: non-zero LI where the oracle has 0"
+    # A material the ray never touches (or a ray that misses) must give exactly zero.  The one exception is the tie of
+    # reading Q9: a midpoint within 2^-12 of a cell face may be sampled in the neighbouring cell, which brings in that
+    # cell's far corners with a weight <= 2^-12; such an entry must be that ray (near_face says so from the oracle's
+    # own positions) and stay below the floor like every other entry.
+    zero_bad = np.argwhere((li_ref == 0.0) & (li_gpu != 0.0))
+    if len(zero_bad):
+        assert near_face is not None and len(zero_bad) <= 1000, \
+            f"{what}: {len(zero_bad)} non-zero LI where the oracle has 0"
+        for index in zero_bad:
+            assert near_face(index), (f"{what}: non-zero LI {li_gpu[tuple(index)]:.3e} at {tuple(index)} where the "
+                                      "oracle has 0, and no sample of that ray is within 2^-12 of a cell face")
     needed_floor = int(np.count_nonzero(err > LI_RTOL * np.abs(li_ref)))
     rel = float((err / np.maximum(np.abs(li_ref), 1e-300))[li_ref > 1e-3 * scale].max()) if scale else 0.0
     return rel, needed_floor
@@ -49,6 +78,7 @@ def compare_full(projector, w, oracle_out, what=""):
     sig, li, tab = projector.project(want_li=True, want_table=True)
     sig, li, tab = sig.cpu().numpy(), li.cpu().numpy(), tab.cpu().numpy()
     check_ray_table(tab, oracle_out["ray_table"], what)
-    worst_li, n_floor = check_line_integrals(li, oracle_out["line_integrals"], what)
+    near_face = face_tie_checker(w, list(range(w.n_proj))) if getattr(w, "poses", None) is None else None
+    worst_li, n_floor = check_line_integrals(li, oracle_out["line_integrals"], what, near_face)
     worst_sig = check_signal(sig, oracle_out["signal"], what)
     return dict(signal=worst_sig, li=worst_li, li_floor_pixels=n_floor)

@@ -22,7 +22,8 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 import oracle  # noqa: E402
-from parity_util import LI_FLOOR, LI_RTOL, check_line_integrals, check_ray_table, check_signal  # noqa: E402
+from parity_util import (LI_FLOOR, LI_RTOL, check_line_integrals, check_ray_table, check_signal,  # noqa: E402
+                         face_tie_checker)
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -46,7 +47,7 @@ def _scan_parity(gdrr, w, name, projections, block, sampler=0, layout=2):
     """Projects `projections` (a list of indices into w's scan) in blocks, runs the oracle on every pixel of each
     block and applies the three checks; returns the record of the worst cases."""
     rec = dict(config=name, sampler=sampler, layout=layout, projections=len(projections), pixels=0, samples=0,
-               ray_table_differences=0, worst_rel_signal=0.0, worst_rel_li=0.0, li_floor_pixels=0,
+               ray_table_differences=0, face_tie_entries=0, worst_rel_signal=0.0, worst_rel_li=0.0, li_floor_pixels=0,
                worst_projection=None, oracle_seconds=0.0, gpu_kernel_launches=0)
     t_start = time.time()
     with gdrr.Projector(w, layout=layout, sampler=sampler) as pr:
@@ -66,7 +67,8 @@ def _scan_parity(gdrr, w, name, projections, block, sampler=0, layout=2):
             rec["oracle_seconds"] += time.time() - t0
             what = f"{name} projections {idx[0]}..{idx[-1]}"
             check_ray_table(tab, ref["ray_table"], what)
-            rel_li, n_floor = check_line_integrals(li, ref["line_integrals"], what)
+            rec["face_tie_entries"] += int(np.count_nonzero((ref["line_integrals"] == 0.0) & (li != 0.0)))
+            rel_li, n_floor = check_line_integrals(li, ref["line_integrals"], what, face_tie_checker(w, idx))
             rel_sig = check_signal(sig, ref["signal"], what)
             rec["pixels"] += int(sig.size)
             rec["samples"] += int(ref["ray_table"][..., 1].sum())

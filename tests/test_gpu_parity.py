@@ -314,8 +314,10 @@ def test_error_codes_on_device(gdrr):
         assert e.value.code == gdrr.GDRR_ERR_NOT_READY
         gdrr.gdrr_set_spectrum(ctx, [1.0], [1.0], [[0.02]])
         with pytest.raises(gdrr.GdrrError) as e:                    # range
-            gdrr.gdrr_project(ctx, vol, 1, 2, sig)
+            gdrr.gdrr_project(ctx, vol, 1, 2, torch.empty((2, 8, 8), dtype=torch.float32, device="cuda"))
         assert e.value.code == gdrr.GDRR_ERR_INVALID_ARG
+        with pytest.raises(ValueError):                             # the binding checks what the C ABI cannot see:
+            gdrr.gdrr_project(ctx, vol, 0, 2, sig)                  # an output tensor smaller than the request
         gdrr.gdrr_project(ctx, vol, 0, 1, sig)
         torch.cuda.synchronize()
         # a material index out of range is caught on the device
