@@ -247,6 +247,28 @@ GDRR_API int gdrr_volume_attach_texture(gdrr_context* ctx, gdrr_volume* vol, voi
  * Errors: INVALID_ARG (unknown value). */
 GDRR_API int gdrr_set_sampler(gdrr_context* ctx, int sampler);
 
+/* Which kernel the last tri-linear gdrr_project / gdrr_project_host launch on ctx used for a PACKED_QUAD volume:
+ * GDRR_SAMPLER_STAGED or GDRR_SAMPLER_GATHER; 0 before the first such launch and after a launch on an exact layout.
+ * (What GDRR_SAMPLER_AUTO picks is part of the measured performance: tests/test_gpu_sampler_choice.py pins it.) */
+GDRR_API int gdrr_last_sampler(const gdrr_context* ctx);
+
+/* ---- test hooks (never needed by a user; SURVEY.md section 5 race evidence, reading Q9) ------------------- */
+
+/* mode != 0 makes the following staged-sampler launches on ctx run a build of the kernel in which every warp sleeps,
+ * before it waits on or signals a barrier of the staging ring, for a time keyed on its number and the chunk:
+ * 1 pseudo-random, 2 always the same warp last, 3 the producer warp late.  The images must not change by a bit.
+ * mode 0 (default) is the product kernel, which contains none of this.  Errors: INVALID_ARG (mode outside 0..3). */
+GDRR_API int gdrr_debug_set_skew(gdrr_context* ctx, int mode);
+
+/* Writes the cell (floor of the index-space position per axis, voxel (ix, iy, iz) = cell whose low corner is that
+ * voxel's centre; -1 in the half-voxel rim) of every midpoint sample of the ray through pixel (i, j) of `projection`,
+ * formed with the position arithmetic of the kernel named by sampler (GDRR_SAMPLER_GATHER or GDRR_SAMPLER_STAGED), into
+ * cells_dev [max_samples][3] int32 (first min(n, max_samples) rows) and the ray's n into *count_dev.  Reading Q9:
+ * these may differ from the oracle's fp64 cells only where a position is within 2^-12 of a cell face.
+ * Asynchronous on cuda_stream.  Errors: INVALID_ARG, NOT_READY as gdrr_project; volume must be PACKED_QUAD. */
+GDRR_API int gdrr_debug_ray_cells(gdrr_context* ctx, const gdrr_volume* vol, int projection, int i, int j, int sampler,
+                         int32_t* cells_dev, int max_samples, int32_t* count_dev, void* cuda_stream);
+
 /* Siddon traversal only: writes, per ray of the range, the number of voxel
  * segments of positive length into n_segments_dev [proj_count][nv][nu] int32
  * (0 for a miss).  Asynchronous on cuda_stream. */

@@ -42,7 +42,7 @@ EXPORTS = (
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
     "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture", "gdrr_denoise_scatter",
-    "gdrr_set_geometry_poses",
+    "gdrr_set_geometry_poses", "gdrr_last_sampler", "gdrr_debug_set_skew", "gdrr_debug_ray_cells",
 )
 
 
@@ -79,6 +79,9 @@ def _load():
         "gdrr_volume_attach_texture": (i, [vp, vp, vp]),
         "gdrr_denoise_scatter": (i, [vp, vp, vp, vp, i, i, i, d, d, i, d, vp]),
         "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
+        "gdrr_last_sampler": (i, [vp]),
+        "gdrr_debug_set_skew": (i, [vp, i]),
+        "gdrr_debug_ray_cells": (i, [vp, vp, i, i, i, i, vp, i, vp, vp]),
         "gdrr_kernel_launches": (ctypes.c_ulonglong, [vp]),
         "gdrr_version": (ctypes.c_char_p, []),
     }
@@ -320,6 +323,21 @@ def gdrr_siddon_segments(ctx, vol, proj_begin, proj_count, n_segments_dev, strea
     _check(_lib.gdrr_siddon_segments(ctx, vol, int(proj_begin), int(proj_count),
                                      _dev(n_segments_dev, "int32", _plane(ctx, proj_count), "n_segments_dev"),
                                      _stream(stream)), ctx)
+
+
+def gdrr_last_sampler(ctx):
+    return int(_lib.gdrr_last_sampler(ctx))
+
+
+def gdrr_debug_set_skew(ctx, mode):
+    _check(_lib.gdrr_debug_set_skew(ctx, int(mode)), ctx)
+
+
+def gdrr_debug_ray_cells(ctx, vol, projection, i, j, sampler, cells_dev, count_dev, stream=None):
+    """cells_dev: int32 CUDA tensor [max_samples][3]; count_dev: int32 CUDA tensor [1]."""
+    _check(_lib.gdrr_debug_ray_cells(ctx, vol, int(projection), int(i), int(j), int(sampler),
+                                     _dev(cells_dev, "int32", 0, "cells_dev"), int(cells_dev.numel() // 3),
+                                     _dev(count_dev, "int32", 1, "count_dev"), _stream(stream)), ctx)
 
 
 def gdrr_kernel_launches(ctx):

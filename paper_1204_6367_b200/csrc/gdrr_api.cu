@@ -45,6 +45,8 @@ struct gdrr_context {
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
     int method = GDRR_METHOD_TRILINEAR;
     int sampler = GDRR_SAMPLER_AUTO;
+    int last_sampler = 0;           // kernel the last tri-linear launch on a PACKED_QUAD volume used (gdrr_last_sampler)
+    unsigned debug_skew = 0;        // gdrr_debug_set_skew
 };
 
 struct gdrr_volume {
@@ -250,6 +252,8 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     P.chunk = chunk;
     P.frac_mask = 0x007FFFFFu;
     P.one_bits = 0x3F800000u;
+    P.debug_skew = ctx->debug_skew;
+    for (int a = 0; a < 3; ++a) P.hull_margin[a] = 0.0;
     return GDRR_OK;
 }
 
@@ -331,23 +335,77 @@ bool beam_fits(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& 
     return ext[0] <= 12.5 && ext[1] <= 12.5 && ext[2] <= 8.9;
 }
 
+// The staged sampler bounds a chunk of a CTA's beam by its four CORNER rays (project_staged.cu).  How far can a ray of
+// the tile lie outside their hull at equal interval index?  Sample k of the ray through detector point (u, v) is
+// x = S + t_k n / |n|, n = D(u, v) - S, D affine in (u, v) with unit steps u_hat, v_hat.  For f = n_a / |n|:
+// f_uu = -2 u_hat_a s / L^2 - n_a / L^3 + 3 n_a s^2 / L^3 with L = |n|, s = (n . u_hat) / L, so |f_uu| <= 6 / L^2, the
+// same for v; bilinear interpolation between the corners of a tile with edges hu, hv is therefore off by at most
+// (hu^2 + hv^2) / 8 * 6 / L_min^2, a bilinear function takes its extremes at the corners, and t_k <= L_max.  In voxels
+// of axis a:  margin_a = 0.75 (hu^2 + hv^2) L_max / (L_min^2 d_a) + 2^-10, the last term for the samplers' fixed-point
+// positions (<= 2^-19) and the fp64 rounding of the producer's own.  L_min = distance of the source from the detector
+// plane, L_max = its distance from the farthest detector corner, both over the requested projections.
+// Returns false if a margin exceeds 0.45 voxel (tiles too wide for the source distance): the caller then gathers.
+bool hull_margins(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& g, double (&margin)[3]) {
+    double lmin = 1e300, lmax = 0.0, h2 = 0.0;
+    const double ue[2] = {(0.0 - g.half_nu) * g.du + g.u_off, ((double)(g.nu - 1) - g.half_nu) * g.du + g.u_off};
+    const double ve[2] = {(0.0 - g.half_nv) * g.dv + g.v_off, ((double)(g.nv - 1) - g.half_nv) * g.dv + g.v_off};
+    for (int p = g.proj_begin; p < g.proj_begin + g.proj_count; ++p) {
+        const double* q = &c->poses[12 * (size_t)p];
+        const double *S = q, *P = q + 3, *uh = q + 6, *vh = q + 9;
+        const double nrm[3] = {uh[1] * vh[2] - uh[2] * vh[1], uh[2] * vh[0] - uh[0] * vh[2], uh[0] * vh[1] - uh[1] * vh[0]};
+        double dist = 0.0, nn = 0.0, uu = 0.0, vv = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            dist += (P[a] - S[a]) * nrm[a];
+            nn += nrm[a] * nrm[a];
+            uu += uh[a] * uh[a];
+            vv += vh[a] * vh[a];
+        }
+        lmin = std::fmin(lmin, std::fabs(dist) / std::sqrt(nn));
+        for (int cu = 0; cu < 2; ++cu)
+            for (int cv = 0; cv < 2; ++cv) {
+                double l2 = 0.0;
+                for (int a = 0; a < 3; ++a) {
+                    const double n = P[a] + ue[cu] * uh[a] + ve[cv] * vh[a] - S[a];
+                    l2 += n * n;
+                }
+                lmax = std::fmax(lmax, std::sqrt(l2));
+            }
+        const double hu = (kTileU - 1) * g.du * std::sqrt(uu), hv = (kStageTileV - 1) * g.dv * std::sqrt(vv);
+        h2 = std::fmax(h2, hu * hu + hv * hv);
+    }
+    bool ok = lmin > 0.0;
+    for (int a = 0; a < 3; ++a) {
+        margin[a] = ok ? 0.75 * h2 * lmax / (lmin * lmin * vol->d[a]) + 1.0 / 1024.0 : 1e300;
+        ok = ok && margin[a] <= 0.45;
+    }
+    return ok;
+}
+
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
-    if (vol->ctx->method == GDRR_METHOD_SIDDON) {
+    gdrr_context* c = vol->ctx;
+    if (c->method == GDRR_METHOD_SIDDON) {
         cudaError_t e = ensure_compact(vol, s);
         if (e != cudaSuccess) return e;
         return launch_project_siddon(P, vol->vw, vol->layout, s);
     }
-    if (vol->ctx->method == GDRR_METHOD_TEXTURE) return launch_project_texture(P, vol->vw, (unsigned long long)vol->tex, s);
-    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && vol->ctx->sampler != GDRR_SAMPLER_GATHER) {
+    if (c->method == GDRR_METHOD_TEXTURE) return launch_project_texture(P, vol->vw, (unsigned long long)vol->tex, s);
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD && vol->has_tmap && c->sampler != GDRR_SAMPLER_GATHER) {
         // AUTO: staging pays when the beam of a 16 x 16-pixel CTA over 16 steps fits the 14 x 14 x 11-quad box
-        // (a chunk that does not fit is gathered anyway, after paying for its bounding box)
-        const gdrr_context* c = vol->ctx;
+        // (a chunk that does not fit is gathered anyway, after its box has been refused)
         const bool fits = beam_fits(c, vol, P.g);
         // (the staged kernel keeps a chunk's base in 5.27 fixed point: 16 steps must advance less than 16 voxels)
         const double adv16 = 16.0 * P.g.step / std::fmin(vol->d[0], std::fmin(vol->d[1], vol->d[2]));
-        if (adv16 <= 15.0 && (fits || c->sampler == GDRR_SAMPLER_STAGED)) return launch_project_staged(P, vol->vw, &vol->tmap, s);
+        ProjectParams Ps = P;
+        if (adv16 <= 15.0 && (fits || c->sampler == GDRR_SAMPLER_STAGED) && hull_margins(c, vol, P.g, Ps.hull_margin)) {
+            c->last_sampler = GDRR_SAMPLER_STAGED;
+            return launch_project_staged(Ps, vol->vw, &vol->tmap, s);
+        }
     }
-    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) return launch_project_packed(P, vol->vw, s);
+    if (vol->layout == GDRR_LAYOUT_PACKED_QUAD) {
+        c->last_sampler = GDRR_SAMPLER_GATHER;
+        return launch_project_packed(P, vol->vw, s);
+    }
+    c->last_sampler = 0;
     return launch_project_exact(P, vol->vw, vol->layout, s);
 }
 
@@ -814,6 +872,35 @@ int gdrr_siddon_segments(gdrr_context* ctx, const gdrr_volume* vol, int proj_beg
     cudaError_t e = ensure_compact(vol, (cudaStream_t)cuda_stream);
     if (e == cudaSuccess) e = launch_project_siddon(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "Siddon kernel launch");
+    ctx->launches += 1;
+    return GDRR_OK;
+}
+
+int gdrr_last_sampler(const gdrr_context* ctx) { return ctx ? ctx->last_sampler : 0; }
+
+int gdrr_debug_set_skew(gdrr_context* ctx, int mode) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (mode < 0 || mode > 3) return fail(ctx, GDRR_ERR_INVALID_ARG, "skew mode must be 0..3 (got %d)", mode);
+    ctx->debug_skew = (unsigned)mode;
+    return GDRR_OK;
+}
+
+int gdrr_debug_ray_cells(gdrr_context* ctx, const gdrr_volume* vol, int projection, int i, int j, int sampler,
+                         int32_t* cells_dev, int max_samples, int32_t* count_dev, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!cells_dev || !count_dev || max_samples < 0) return fail(ctx, GDRR_ERR_INVALID_ARG, "an output is NULL");
+    if (sampler != GDRR_SAMPLER_GATHER && sampler != GDRR_SAMPLER_STAGED)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "sampler must be GDRR_SAMPLER_GATHER or GDRR_SAMPLER_STAGED");
+    ProjectParams P;
+    int rc = fill_project(ctx, vol, projection, 1, P);
+    if (rc) return rc;
+    if (vol->layout != GDRR_LAYOUT_PACKED_QUAD) return fail(ctx, GDRR_ERR_INVALID_ARG, "the volume is not PACKED_QUAD");
+    if (i < 0 || i >= ctx->nu || j < 0 || j >= ctx->nv) return fail(ctx, GDRR_ERR_INVALID_ARG, "pixel outside the detector");
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    cudaError_t e = launch_debug_ray_cells(P, i, j, sampler == GDRR_SAMPLER_STAGED, cells_dev, max_samples, count_dev,
+                                           (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "debug kernel launch");
     ctx->launches += 1;
     return GDRR_OK;
 }

@@ -11,16 +11,13 @@ namespace gdrr {
 constexpr int kTileU = 16;
 constexpr int kTileV = 16;
 constexpr int kThreads = kTileU * kTileV;
-// staged sampler: its own CTA tile and staging box (project_staged.cu; the tensor map is made in gdrr_api.cu)
+// staged sampler (project_staged.cu; the tensor map is made in gdrr_api.cu): the same 16 x 16 tile sampled by 8 consumer
+// warps, plus one producer warp; two staged boxes of kBX x kBY x kBZ quads; 3 CTAs per SM
 // (measured on C3: a 16 x 8 tile with a 14 x 14 x 7 box, 4 CTAs per SM: -8%)
-#ifndef GDRR_STAGE_TILE_V
-#define GDRR_STAGE_TILE_V 16
-#define GDRR_STAGE_BOX_Z 11
 #define GDRR_STAGE_CTAS 3
-#endif
-constexpr int kStageTileV = GDRR_STAGE_TILE_V;
+constexpr int kStageTileV = 16;
 constexpr int kStageThreads = kTileU * kStageTileV;
-constexpr int kBX = 14, kBY = 14, kBZ = GDRR_STAGE_BOX_Z;       // box, in quads
+constexpr int kBX = 14, kBY = 14, kBZ = 11;       // box, in quads
 constexpr int kMaxChunk = 32;       // samples between two fp64 re-bases of the position
 constexpr int kFracBits = 23;       // fixed-point fraction bits of the in-chunk position
 
@@ -59,6 +56,11 @@ struct ProjectParams {
     int n_energy, n_mat;
     int chunk;                      // <= kMaxChunk
     unsigned frac_mask, one_bits;   // 0x007FFFFF, 0x3F800000: kept in registers by the samplers
+    // staged sampler: bound, in voxels per axis, on how far a ray of a 16 x 16-pixel tile can lie outside the hull of
+    // the tile's four corner rays at equal interval index (curvature of the equal-index surface plus the
+    // fixed-point slack of the sampler's positions); gdrr_api.cu hull_margins()
+    double hull_margin[3];
+    unsigned debug_skew;            // tests only (gdrr_debug_set_skew): forced warp orders in the staged kernel, 0 = off
     float* signal;                  // [proj_count][nv][nu]
     float* li;                      // [proj_count][n_mat][nv][nu] or nullptr
     int32_t* ray_table;             // [proj_count][nv][nu][2] or nullptr
@@ -84,10 +86,14 @@ cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_
 cudaError_t launch_compact_copy(const IngestParams& p, cudaStream_t s);
 cudaError_t launch_project_exact(const ProjectParams& p, int vw, int layout, cudaStream_t s);
 cudaError_t launch_project_packed(const ProjectParams& p, int vw, cudaStream_t s);
-// tensor_map: a CUtensorMap over the packed-quad volume (3-D: words along x, rows, slabs; box 4*14 x 14 x 11)
+// tensor_map: a CUtensorMap over the packed-quad volume (3-D: words along x, rows, slabs; box 4*14 x 14 x 11);
+// launches kStageThreads + 32 threads per CTA (the consumer warps and the producer warp)
 cudaError_t launch_project_staged(const ProjectParams& p, int vw, const void* tensor_map, cudaStream_t s);
 cudaError_t launch_project_texture(const ProjectParams& p, int vw, unsigned long long tex_object, cudaStream_t s);
 cudaError_t launch_project_siddon(const ProjectParams& p, int vw, int layout, cudaStream_t s);
+// tests only: cells of every sample of ray (i, j) of projection p.g.proj_begin as the staged (or gather) kernel forms them
+cudaError_t launch_debug_ray_cells(const ProjectParams& p, int i, int j, int staged, int32_t* cells, int max_samples,
+                                   int32_t* count, cudaStream_t s);
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 

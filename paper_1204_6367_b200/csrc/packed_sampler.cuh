@@ -80,56 +80,132 @@ __device__ __forceinline__ int elem_index(int cx, int cy, int cz, int sy, int sz
     return cz * sz + cy * sy + cx;
 }
 
-// UNI: every lane of the warp is here (unpredicated chunk): vote, so that the common case "all lanes
-// in a pure cell of their running material" is a warp-uniform branch without reconvergence overhead.
-template <int VW, bool UNI>
-__device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, float fx, float fy, float fz,
-                                             float& cur, unsigned& curm4, float (&part)[VW]) {
-    bool fast = true;
-    if (VW > 1) fast = (a.x & 7u) == curm4;        // pure cell of the running material
-    if (VW > 1 && UNI) {
-        if (__all_sync(0xffffffffu, fast)) {
-            cur += blend_cell(a, c, fx, fy, fz);
-            return;
-        }
+// State of one ray while it is sampled.  Three levels of sums keep the fp32 accumulation short: `cur` (this chunk's
+// pure cells of the running material), `run` (the ray's total for the running material since it last changed),
+// `part` (this chunk's mixed cells and closed runs, per material; `dirty` says it was touched).
+template <int VW>
+struct RayAcc {
+    float part[VW];     // per-material partial sums of the current chunk
+    float cur;          // this chunk's sum of pure cells of material curm4 & 3
+    float run;          // the same over the earlier chunks since the running material last changed
+    unsigned curm4;     // 4 | running material
+    bool dirty;         // part[] is not all zero (warp-uniform)
+};
+
+// The running sum moves to material m4 (4 | material): what it held goes to its old material.
+template <int VW>
+__device__ __forceinline__ void switch_material(RayAcc<VW>& A, unsigned m4) {
+    add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur + A.run);
+    A.cur = 0.f;
+    A.run = 0.f;
+    A.curm4 = m4;
+}
+
+// A cell that is not a pure cell of the running material; v = blend_cell(a, c, fx, fy, fz) of all 8 words.
+// Tags of the first element a (volume_layout.cu): a.x bit 2 "all 8 corners have the material of a.x"; a.y bit 2 "the 8
+// corners have exactly two materials", the second one in (a.w bit 2, a.z bit 2).
+template <int VW>
+__device__ __forceinline__ void blend_general(const uint4& a, const uint4& c, float fx, float fy, float fz, float v,
+                                              RayAcc<VW>& A) {
+    if (a.x & 4u) {
+        // pure cell of another material: the running sum moves there
+        switch_material<VW>(A, a.x & 7u);
+        A.cur = v;
+        return;
     }
-    if (fast) {
-        cur += blend_cell(a, c, fx, fy, fz);
+    const unsigned p = a.x & 3u;
+    if (a.y & 4u) {
+        // two materials p and q: one more blend of the corners of material p alone (the others as 0), the rest is q's
+        uint4 ma, mc;
+        ma.x = a.x;
+        ma.y = ((a.y ^ p) & 3u) ? 0u : a.y;
+        ma.z = ((a.z ^ p) & 3u) ? 0u : a.z;
+        ma.w = ((a.w ^ p) & 3u) ? 0u : a.w;
+        mc.x = ((c.x ^ p) & 3u) ? 0u : c.x;
+        mc.y = ((c.y ^ p) & 3u) ? 0u : c.y;
+        mc.z = ((c.z ^ p) & 3u) ? 0u : c.z;
+        mc.w = ((c.w ^ p) & 3u) ? 0u : c.w;
+        const float vp = blend_cell(ma, mc, fx, fy, fz);
+        const unsigned q = ((a.z >> 2) & 1u) | ((a.w >> 1) & 2u);
+        add_routed<VW>(A.part, (int)p, vp);
+        add_routed<VW>(A.part, (int)q, v - vp);
     } else {
-        // mixed cell, or a pure cell of another material: route every weighted corner
+        // three or four materials: route every weighted corner
         const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
         const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
         // w<y><z>; words (x0y0, x0y1, x1y0, x1y1)
-        add_routed<VW>(part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
-        add_routed<VW>(part, (int)(a.y & 3u), gx * w10 * __uint_as_float(a.y));
-        add_routed<VW>(part, (int)(a.z & 3u), fx * w00 * __uint_as_float(a.z));
-        add_routed<VW>(part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
-        add_routed<VW>(part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
-        add_routed<VW>(part, (int)(c.y & 3u), gx * w11 * __uint_as_float(c.y));
-        add_routed<VW>(part, (int)(c.z & 3u), fx * w01 * __uint_as_float(c.z));
-        add_routed<VW>(part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
-        // the running sum follows the material the ray is now in
-        const unsigned m4 = (c.w & 3u) | 4u;
-        if (m4 != curm4) {
-            add_routed<VW>(part, (int)(curm4 & 3u), cur);
-            cur = 0.f;
-            curm4 = m4;
+        add_routed<VW>(A.part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
+        add_routed<VW>(A.part, (int)(a.y & 3u), gx * w10 * __uint_as_float(a.y));
+        add_routed<VW>(A.part, (int)(a.z & 3u), fx * w00 * __uint_as_float(a.z));
+        add_routed<VW>(A.part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
+        add_routed<VW>(A.part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
+        add_routed<VW>(A.part, (int)(c.y & 3u), gx * w11 * __uint_as_float(c.y));
+        add_routed<VW>(A.part, (int)(c.z & 3u), fx * w01 * __uint_as_float(c.z));
+        add_routed<VW>(A.part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
+    }
+    // the running sum follows the material the ray is now in
+    const unsigned m4 = (c.w & 3u) | 4u;
+    if (m4 != A.curm4) switch_material<VW>(A, m4);
+}
+
+// One sample.  UNI: every lane of the warp is here (unpredicated chunk): vote, so that the common case "all lanes
+// in a pure cell of their running material" is a warp-uniform branch without reconvergence overhead.
+template <int VW, bool UNI>
+__device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, float fx, float fy, float fz,
+                                             RayAcc<VW>& A) {
+    const float v = blend_cell(a, c, fx, fy, fz);
+    if (VW == 1) {
+        A.cur += v;
+        return;
+    }
+    const bool fast = (a.x & 7u) == A.curm4;        // pure cell of the running material
+    if (UNI) {
+        if (__all_sync(0xffffffffu, fast)) {
+            A.cur += v;
+            return;
         }
     }
+    A.dirty = true;
+    if (fast) A.cur += v;
+    else blend_general<VW>(a, c, fx, fy, fz, v, A);
+}
+
+// End of a chunk: the chunk's sums move up one level (see RayAcc).
+template <int VW>
+__device__ __forceinline__ void flush_chunk(RayAcc<VW>& A, float (&acc)[VW]) {
+    A.run += A.cur;
+    A.cur = 0.f;
+    if (VW > 1 && A.dirty) {
+#pragma unroll
+        for (int k = 0; k < VW; ++k) {
+            acc[k] += A.part[k];
+            A.part[k] = 0.f;
+        }
+        A.dirty = false;
+    }
+}
+
+// End of the ray: the running material's total joins the others.
+template <int VW>
+__device__ __forceinline__ void finish_ray(RayAcc<VW>& A, float (&acc)[VW]) {
+    if (VW == 1) acc[0] += A.run;
+    else add_routed<VW>(acc, (int)(A.curm4 & 3u), A.run);
+}
+
+template <int VW>
+__device__ __forceinline__ void init_ray(RayAcc<VW>& A) {
+#pragma unroll
+    for (int k = 0; k < VW; ++k) A.part[k] = 0.f;
+    A.cur = 0.f;
+    A.run = 0.f;
+    A.curm4 = 4u;
+    A.dirty = false;
 }
 
 // element of the sample at in-chunk fixed-point position q (idx0 = element of the chunk's base cell)
 __device__ __forceinline__ int sample_index(int idx0, int qx, int qy, int qz, int sy, int sz) {
     return idx0 + (qz >> kFracBits) * sz + (qy >> kFracBits) * sy + (qx >> kFracBits);
 }
-
-// State of one ray while it is sampled.
-template <int VW>
-struct RayAcc {
-    float part[VW];     // per-material partial sums of the current chunk
-    float cur;          // running sum of pure cells of material curm4 & 3
-    unsigned curm4;     // 4 | material
-};
 
 struct Sampler {
     const uint4* __restrict__ vol0;     // slab iz
@@ -167,7 +243,7 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
             a1 = __ldg(S.vol0 + idx);
             c1 = __ldg(S.vol1 + idx);
         }
-        if (act0) blend_sample<VW, !PRED>(a0, c0, fx, fy, fz, A.cur, A.curm4, A.part);
+        if (act0) blend_sample<VW, !PRED>(a0, c0, fx, fy, fz, A);
         if (more) {
             fx = frac_float(qx, S.fmask, S.fone);
             fy = frac_float(qy, S.fmask, S.fone);
@@ -180,8 +256,38 @@ __device__ __forceinline__ void run_chunk(const Sampler& S, const ChunkBase& b, 
                 a0 = __ldg(S.vol0 + idx);
                 c0 = __ldg(S.vol1 + idx);
             }
-            if (act1) blend_sample<VW, !PRED>(a1, c1, fx, fy, fz, A.cur, A.curm4, A.part);
+            if (act1) blend_sample<VW, !PRED>(a1, c1, fx, fy, fz, A);
         }
+    }
+}
+
+// Chunk bases of the staged sampler.  The position of a chunk's first sample is (cell cb, fraction qb in 2^-27 voxel);
+// the next chunk's is that plus D = round(kStageK dg 2^27), in integers.  The fp64 line of the ray is used once, for the
+// CTA's first chunk: the base then drifts by <= 2^-28 voxel per chunk (2^-19 over the 500 chunks of the longest ray a
+// 180 GB volume allows), and 12 registers of doubles do not live through the loop.  Inside a chunk the samples step by
+// dq = round(dg 2^23) from the base's 23-bit fraction.
+constexpr int kStageK = 16;                       // interval indices per staged chunk
+constexpr int kBaseBits = 27;                     // fraction bits of a chunk's base position (5.27 fixed point)
+struct ChunkWalk {
+    int cb[3], qb[3], D[3];
+};
+__device__ __forceinline__ void walk_init(const double (&gs)[3], const double (&dg)[3], int first_chunk, ChunkWalk& W) {
+    const double tk = (double)(first_chunk * kStageK) + 0.5;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double x = fma(tk, dg[a], gs[a]);
+        const double f = floor(x);
+        W.cb[a] = (int)f;
+        W.qb[a] = (int)((x - f) * (double)(1 << kBaseBits));
+        W.D[a] = __double2int_rn(dg[a] * (double)kStageK * (double)(1 << kBaseBits));
+    }
+}
+__device__ __forceinline__ void walk_advance(ChunkWalk& W) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int q = W.qb[a] + W.D[a];
+        W.cb[a] += q >> kBaseBits;
+        W.qb[a] = q & ((1 << kBaseBits) - 1);
     }
 }
 
@@ -213,8 +319,8 @@ __device__ __forceinline__ void run_chunk_pairs(const Sampler& S, const ChunkBas
             A.cur += blend_cell(a0, c0, fx0, fy0, fz0);
             A.cur += blend_cell(a1, c1, fx1, fy1, fz1);
         } else {
-            blend_sample<VW, false>(a0, c0, fx0, fy0, fz0, A.cur, A.curm4, A.part);
-            blend_sample<VW, false>(a1, c1, fx1, fy1, fz1, A.cur, A.curm4, A.part);
+            blend_sample<VW, false>(a0, c0, fx0, fy0, fz0, A);
+            blend_sample<VW, false>(a1, c1, fx1, fy1, fz1, A);
         }
     }
 }

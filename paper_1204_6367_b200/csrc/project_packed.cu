@@ -91,8 +91,7 @@ gdrr_project_packed_kernel(const ProjectParams P) {
 #pragma unroll
     for (int m = 0; m < VW; ++m) acc[m] = 0.f;
     RayAcc<VW> A;
-    A.cur = 0.f;
-    A.curm4 = 4u;
+    init_ray<VW>(A);
 
     for (int kc = (kmin / CH) * CH; kc < kmax; kc += CH) {
         const int s0 = max(kmin - kc, 0);
@@ -105,20 +104,15 @@ gdrr_project_packed_kernel(const ProjectParams P) {
         }
         const ChunkBase b = chunk_base(gs, dg, kc + s0);
         const unsigned rel = (unsigned)(kc + s0 - j0);
-#pragma unroll
-        for (int m = 0; m < VW; ++m) A.part[m] = 0.f;
-
         const bool mine = rel < un && rel + (unsigned)cnt <= un;         // this lane owns the whole chunk
         if (__all_sync(0xffffffffu, mine) && !(cnt & 1))
             run_chunk_pairs<VW>(S, b, cnt, A);
         else
             run_chunk<VW, true>(S, b, cnt, rel, un, A);
 
-        add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur);
-        A.cur = 0.f;
-#pragma unroll
-        for (int m = 0; m < VW; ++m) acc[m] += A.part[m];
+        flush_chunk<VW>(A, acc);
     }
+    finish_ray<VW>(A, acc);
 
     if (valid) finish_pixel<VW>(P, s_mu, s_src, acc, P.g.step, pl, i, j);
 }

@@ -65,9 +65,11 @@ gdrr_ingest_kernel(const IngestParams P) {
 // PACKED_QUAD (project_packed.cu): element (ex, ey, ez) = the four words of stored
 // voxels (ex, ey), (ex, ey+1), (ex+1, ey), (ex+1, ey+1) of slab ez.  With more than
 // one material a word is rho rounded to a 21-bit mantissa with tags in the three
-// freed bits: bits 0-1 the material index; bit 2, in the first word of an element
-// only, "the 8 corners of cell (ex, ey, ez) (this quad and the one above it in slab
-// ez + 1) all have this material".  Elements are stored linearly with strides sy, sz.
+// freed bits: bits 0-1 the material index; bit 2 describes cell (ex, ey, ez), whose 8
+// corners are this quad and the one above it in slab ez + 1: in the first word "all 8
+// corners have this material"; in the second word "the 8 corners have exactly two
+// materials", the one that is not the first word's then in bit 2 of the fourth (its
+// bit 1) and third (its bit 0) words.  Elements are stored linearly with strides sy, sz.
 // One thread per element slot; slots that are stride padding are zeroed.  Grid: x over a row's sy slots
 // (+ the few pad slots between the last row and the slab pitch, taken by the blocks of the last row),
 // y = row, z = slab: no division in the index arithmetic.
@@ -81,7 +83,7 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
     uint4 out = make_uint4(0u, 0u, 0u, 0u);
     if (ex < P.px && ey < P.py) {
         unsigned w[4];
-        unsigned mixed = 0u, m0 = 0u;
+        unsigned mixed = 0u, m0 = 0u, seen = 0u;        // seen: bit m set if a corner has material m
 #pragma unroll
         for (int dz = 0; dz < 2; ++dz) {
             const int iz = min(max(ez + dz - 1, 0), P.nz - 1);
@@ -93,6 +95,7 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
                 const unsigned m = P.mat[src];
                 if (dz == 0 && k == 0) m0 = m;
                 mixed |= m ^ m0;
+                seen |= 1u << (m & 3u);
                 if (dz == 0) {
                     unsigned bits = __float_as_uint(P.rho[src]);
                     if ((int)m >= P.n_mat) *P.bad_flag = 1;
@@ -102,6 +105,12 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
             }
         }
         if (P.n_mat > 1 && mixed == 0u) w[0] |= 4u;
+        if (P.n_mat > 1 && __popc(seen) == 2) {
+            const unsigned q = (unsigned)(__ffs((int)(seen & ~(1u << (m0 & 3u)))) - 1);     // the other material
+            w[1] |= 4u;
+            w[2] |= (q & 1u) << 2;
+            w[3] |= (q & 2u) << 1;
+        }
         out = make_uint4(w[0], w[1], w[2], w[3]);
     }
     reinterpret_cast<uint4*>(P.vox)[o] = out;
