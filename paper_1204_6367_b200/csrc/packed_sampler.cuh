@@ -80,22 +80,28 @@ __device__ __forceinline__ int elem_index(int cx, int cy, int cz, int sy, int sz
     return cz * sz + cy * sy + cx;
 }
 
-// State of one ray while it is sampled.  Three levels of sums keep the fp32 accumulation short: `cur` (this chunk's
-// pure cells of the running material), `run` (the ray's total for the running material since it last changed),
-// `part` (this chunk's mixed cells and closed runs, per material; `dirty` says it was touched).
+// State of one ray while it is sampled.  Three levels of sums keep the fp32 accumulation short and the registers few:
+// `cur` (this chunk's pure cells of the running material), `run` (the ray's total for the running material since it
+// last changed), and the ray's per-material totals of everything else (mixed cells, closed runs) in SHARED memory:
+// slot[m * kAccStride] is this thread's sum for material m (its own bank; only this thread touches it).
+constexpr int kAccStride = kThreads;
 template <int VW>
 struct RayAcc {
-    float part[VW];     // per-material partial sums of the current chunk
     float cur;          // this chunk's sum of pure cells of material curm4 & 3
     float run;          // the same over the earlier chunks since the running material last changed
     unsigned curm4;     // 4 | running material
-    bool dirty;         // part[] is not all zero (warp-uniform)
+    float* slot;        // shared memory: slot[m * kAccStride] += values routed to material m
 };
+
+template <int VW>
+__device__ __forceinline__ void route(RayAcc<VW>& A, unsigned m, float v) {
+    A.slot[m * kAccStride] += v;
+}
 
 // The running sum moves to material m4 (4 | material): what it held goes to its old material.
 template <int VW>
 __device__ __forceinline__ void switch_material(RayAcc<VW>& A, unsigned m4) {
-    add_routed<VW>(A.part, (int)(A.curm4 & 3u), A.cur + A.run);
+    route<VW>(A, A.curm4 & 3u, A.cur + A.run);
     A.cur = 0.f;
     A.run = 0.f;
     A.curm4 = m4;
@@ -127,21 +133,21 @@ __device__ __forceinline__ void blend_general(const uint4& a, const uint4& c, fl
         mc.w = ((c.w ^ p) & 3u) ? 0u : c.w;
         const float vp = blend_cell(ma, mc, fx, fy, fz);
         const unsigned q = ((a.z >> 2) & 1u) | ((a.w >> 1) & 2u);
-        add_routed<VW>(A.part, (int)p, vp);
-        add_routed<VW>(A.part, (int)q, v - vp);
+        route<VW>(A, p, vp);
+        route<VW>(A, q, v - vp);
     } else {
         // three or four materials: route every weighted corner
         const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
         const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
         // w<y><z>; words (x0y0, x0y1, x1y0, x1y1)
-        add_routed<VW>(A.part, (int)(a.x & 3u), gx * w00 * __uint_as_float(a.x));
-        add_routed<VW>(A.part, (int)(a.y & 3u), gx * w10 * __uint_as_float(a.y));
-        add_routed<VW>(A.part, (int)(a.z & 3u), fx * w00 * __uint_as_float(a.z));
-        add_routed<VW>(A.part, (int)(a.w & 3u), fx * w10 * __uint_as_float(a.w));
-        add_routed<VW>(A.part, (int)(c.x & 3u), gx * w01 * __uint_as_float(c.x));
-        add_routed<VW>(A.part, (int)(c.y & 3u), gx * w11 * __uint_as_float(c.y));
-        add_routed<VW>(A.part, (int)(c.z & 3u), fx * w01 * __uint_as_float(c.z));
-        add_routed<VW>(A.part, (int)(c.w & 3u), fx * w11 * __uint_as_float(c.w));
+        route<VW>(A, a.x & 3u, gx * w00 * __uint_as_float(a.x));
+        route<VW>(A, a.y & 3u, gx * w10 * __uint_as_float(a.y));
+        route<VW>(A, a.z & 3u, fx * w00 * __uint_as_float(a.z));
+        route<VW>(A, a.w & 3u, fx * w10 * __uint_as_float(a.w));
+        route<VW>(A, c.x & 3u, gx * w01 * __uint_as_float(c.x));
+        route<VW>(A, c.y & 3u, gx * w11 * __uint_as_float(c.y));
+        route<VW>(A, c.z & 3u, fx * w01 * __uint_as_float(c.z));
+        route<VW>(A, c.w & 3u, fx * w11 * __uint_as_float(c.w));
     }
     // the running sum follows the material the ray is now in
     const unsigned m4 = (c.w & 3u) | 4u;
@@ -165,41 +171,40 @@ __device__ __forceinline__ void blend_sample(const uint4& a, const uint4& c, flo
             return;
         }
     }
-    A.dirty = true;
     if (fast) A.cur += v;
     else blend_general<VW>(a, c, fx, fy, fz, v, A);
 }
 
-// End of a chunk: the chunk's sums move up one level (see RayAcc).
+// End of a chunk: the chunk's sum moves up one level (see RayAcc).
 template <int VW>
-__device__ __forceinline__ void flush_chunk(RayAcc<VW>& A, float (&acc)[VW]) {
+__device__ __forceinline__ void flush_chunk(RayAcc<VW>& A) {
     A.run += A.cur;
     A.cur = 0.f;
-    if (VW > 1 && A.dirty) {
-#pragma unroll
-        for (int k = 0; k < VW; ++k) {
-            acc[k] += A.part[k];
-            A.part[k] = 0.f;
-        }
-        A.dirty = false;
-    }
 }
 
-// End of the ray: the running material's total joins the others.
+// `slot`: this thread's first slot of a [4][kAccStride] float array in shared memory (not needed for one material).
 template <int VW>
-__device__ __forceinline__ void finish_ray(RayAcc<VW>& A, float (&acc)[VW]) {
-    if (VW == 1) acc[0] += A.run;
-    else add_routed<VW>(acc, (int)(A.curm4 & 3u), A.run);
-}
-
-template <int VW>
-__device__ __forceinline__ void init_ray(RayAcc<VW>& A) {
-#pragma unroll
-    for (int k = 0; k < VW; ++k) A.part[k] = 0.f;
+__device__ __forceinline__ void init_ray(RayAcc<VW>& A, float* slot) {
     A.cur = 0.f;
     A.run = 0.f;
     A.curm4 = 4u;
-    A.dirty = false;
+    A.slot = slot;
+    if (VW > 1) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) slot[k * kAccStride] = 0.f;
+    }
+}
+
+// End of the ray: the per-material totals, with the running material's total added to its own.
+template <int VW>
+__device__ __forceinline__ void finish_ray(RayAcc<VW>& A, float (&acc)[VW]) {
+    if (VW == 1) {
+        acc[0] = A.run;
+        return;
+    }
+    route<VW>(A, A.curm4 & 3u, A.run);
+#pragma unroll
+    for (int k = 0; k < VW; ++k) acc[k] = A.slot[k * kAccStride];
 }
 
 // element of the sample at in-chunk fixed-point position q (idx0 = element of the chunk's base cell)

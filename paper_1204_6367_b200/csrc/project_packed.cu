@@ -38,6 +38,7 @@ gdrr_project_packed_kernel(const ProjectParams P) {
     // the ray's line in index space (6 doubles) is needed once per chunk only: keep it in
     // shared memory, not in 12 registers of the sampling loop
     __shared__ double s_line[6][kThreads];
+    __shared__ float s_acc[4][kAccStride];          // per-material sums of the rays (RayAcc)
     float4* s_mu;
     float2* s_src;
     load_tables(P, s_mu, s_src);
@@ -88,10 +89,8 @@ gdrr_project_packed_kernel(const ProjectParams P) {
 
     // ---- a2-a4: sampling -------------------------------------------------------
     float acc[VW];
-#pragma unroll
-    for (int m = 0; m < VW; ++m) acc[m] = 0.f;
     RayAcc<VW> A;
-    init_ray<VW>(A);
+    init_ray<VW>(A, &s_acc[0][threadIdx.x]);
 
     for (int kc = (kmin / CH) * CH; kc < kmax; kc += CH) {
         const int s0 = max(kmin - kc, 0);
@@ -110,7 +109,7 @@ gdrr_project_packed_kernel(const ProjectParams P) {
         else
             run_chunk<VW, true>(S, b, cnt, rel, un, A);
 
-        flush_chunk<VW>(A, acc);
+        flush_chunk<VW>(A);
     }
     finish_ray<VW>(A, acc);
 

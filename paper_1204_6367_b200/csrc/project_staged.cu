@@ -42,37 +42,41 @@ static_assert(kStageThreads % 128 == 0, "the lane -> pixel map below is 4 warps 
 
 __device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count));
+// mbarrier operations on the 32-bit shared-window address of the barrier (formed once per kernel: taking it anew at
+// every use costs six instructions)
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// (try_wait has acquire semantics, arrive has release semantics, both at CTA scope: the PTX defaults)
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+// (try_wait has acquire semantics, arrive has release semantics, both at CTA scope: the PTX defaults.  The last operand
+// is the time, in ns, the hardware may keep the warp suspended before try_wait returns false: long, so that a waiting
+// warp sleeps instead of spinning through issue slots)
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
-        "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+        "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 // box of the 3-D tensor (words along x, rows, slabs) at (c0, c1, c2) -> shared memory, completes on `bar`
-__device__ __forceinline__ void tma_load_box(void* dst, const CUtensorMap* map, int c0, int c1, int c2,
-                                             unsigned long long* bar) {
+__device__ __forceinline__ void tma_load_box(void* dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned bar) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-        ::"r"(smem_addr(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_addr(bar)) : "memory");
+        ::"r"(smem_addr(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
 
-// The quads of the staged boxes (2 stages), then the spectrum tables.
+// The quads of the staged boxes (2 stages), the rays' per-material sums (RayAcc), then the spectrum tables.
 extern __shared__ __align__(128) uint4 s_box[];
+constexpr int kAccBytes = 4 * kAccStride * (int)sizeof(float);
 
 // `cnt` consecutive samples of a chunk out of the staged box: as run_chunk (packed_sampler.cuh),
 // the element index is relative to the box and both slabs of a cell are read with one address.
@@ -177,17 +181,19 @@ template <int VW, bool SKEW>
 __global__ void __launch_bounds__(kStageCtaThreads, GDRR_STAGE_CTAS)
 gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtensorMap tmap) {
     __shared__ StageCtl ctl;
-    float4* s_mu = reinterpret_cast<float4*>(s_box + 2 * kStageElems);
+    float* s_acc = reinterpret_cast<float*>(s_box + 2 * kStageElems);
+    float4* s_mu = reinterpret_cast<float4*>(s_box + 2 * kStageElems + kAccBytes / 16);
     float2* s_src = reinterpret_cast<float2*>(s_mu + P.n_energy);
+    const unsigned bar_full = smem_addr(&ctl.full[0]), bar_empty = smem_addr(&ctl.empty[0]);     // [st]: + 8 st
     for (int e = threadIdx.x; e < P.n_energy; e += kStageCtaThreads) {
         s_mu[e] = P.mu_tab[e];
         s_src[e] = P.src_tab[e];
     }
     if (threadIdx.x == 0) {
-        mbar_init(&ctl.full[0], 1);
-        mbar_init(&ctl.full[1], 1);
-        mbar_init(&ctl.empty[0], kConsumerWarps);
-        mbar_init(&ctl.empty[1], kConsumerWarps);
+        mbar_init(bar_full, 1);
+        mbar_init(bar_full + 8u, 1);
+        mbar_init(bar_empty, kConsumerWarps);
+        mbar_init(bar_empty + 8u, kConsumerWarps);
         ctl.krange[0] = 0x7fffffff;
         ctl.krange[1] = (int)0x80000000;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -195,7 +201,8 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
     }
     __syncthreads();
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // (the warp number through a shuffle: the compiler then knows that the role branches below are warp-uniform)
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const bool producer = warp == kConsumerWarps;
     const int pl = blockIdx.z;
     // consumer: a warp is 4 (u) x 8 (v) pixels (thread_pixel_map), the CTA's tile kTileU x kStageTileV.
@@ -259,17 +266,17 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             const bool fit = mx[0] - mn[0] + 1 <= kBX && mx[1] - mn[1] + 1 <= kBY && mx[2] - mn[2] + 2 <= kBZ;
             skew_delay<SKEW>(8u + (unsigned)m, P.debug_skew);
             // stage st is free once every consumer warp has finished chunk m - 2
-            if (m >= 2) mbar_wait(&ctl.empty[st], (unsigned)((m >> 1) - 1) & 1u);
+            if (m >= 2) mbar_wait(bar_empty + 8u * st, (unsigned)((m >> 1) - 1) & 1u);
             if (lane == 0) {
                 ctl.fit[st] = fit;
                 // element of cell (cx, cy, cz) in the stage: lin + (cz kBY + cy) kBX + cx
                 ctl.lin[st] = st * kStageElems - ((mn[2] * kBY + mn[1]) * kBX + mn[0]);
                 // the phase of full[st] completes either way; its release / acquire orders fit and lin before their readers
                 if (fit) {
-                    mbar_arrive_expect_tx(&ctl.full[st], kBoxBytes);
-                    tma_load_box(s_box + st * kStageElems, &tmap, 4 * mn[0], mn[1], mn[2], &ctl.full[st]);
+                    mbar_arrive_expect_tx(bar_full + 8u * st, kBoxBytes);
+                    tma_load_box(s_box + st * kStageElems, &tmap, 4 * mn[0], mn[1], mn[2], bar_full + 8u * st);
                 } else {
-                    mbar_arrive(&ctl.full[st]);
+                    mbar_arrive(bar_full + 8u * st);
                 }
             }
             __syncwarp();
@@ -290,10 +297,8 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
     const unsigned un = (unsigned)n;
 
     float acc[VW];
-#pragma unroll
-    for (int m = 0; m < VW; ++m) acc[m] = 0.f;
     RayAcc<VW> A;
-    init_ray<VW>(A);
+    init_ray<VW>(A, s_acc + threadIdx.x);
 
     if (nchunks > 0) {
         ChunkWalk W;                                 // base position of the current chunk (packed_sampler.cuh)
@@ -311,7 +316,7 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             const int bcx = W.cb[0], bcy = W.cb[1], bcz = W.cb[2];
             walk_advance(W);
             skew_delay<SKEW>((unsigned)(warp + 3 * m), P.debug_skew);
-            mbar_wait(&ctl.full[st], (unsigned)(m >> 1) & 1u);      // box landed (or: chunk does not fit); fit / lin valid
+            mbar_wait(bar_full + 8u * st, (unsigned)(m >> 1) & 1u);      // box landed (or: chunk does not fit); fit / lin valid
             const bool all_mine = m >= m_lo && m < m_hi;
             const int r = (c_begin + m) * kStageK - j0;         // the chunk's first index in this ray's own count
             const unsigned rel = (unsigned)r;
@@ -331,8 +336,8 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             }
             // this warp is done with stage st
             __syncwarp();
-            if (lane == 0) mbar_arrive(&ctl.empty[st]);
-            flush_chunk<VW>(A, acc);
+            if (lane == 0) mbar_arrive(bar_empty + 8u * st);
+            flush_chunk<VW>(A);
         }
     }
     finish_ray<VW>(A, acc);
@@ -343,10 +348,10 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
 template <int VW, bool SKEW>
 static cudaError_t launch_staged_t(const ProjectParams& p, const CUtensorMap& map, cudaStream_t s) {
     dim3 grid((p.g.nu + kTileU - 1) / kTileU, (p.g.nv + kStageTileV - 1) / kStageTileV, p.g.proj_count);
-    const size_t smem = 2 * (size_t)kStageElems * 16 + (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
+    const size_t smem = 2 * (size_t)kStageElems * 16 + kAccBytes + (size_t)p.n_energy * (sizeof(float4) + sizeof(float2));
     // per device and cheap: set at every launch (the boxes alone exceed the 48 KB default)
     cudaError_t e = cudaFuncSetAttribute(gdrr_project_staged_kernel<VW, SKEW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         2 * kStageElems * 16 + 512 * 24 /* GDRR_MAX_ENERGIES bins */);
+                                         2 * kStageElems * 16 + kAccBytes + 512 * 24 /* GDRR_MAX_ENERGIES bins */);
     if (e != cudaSuccess) return e;
     gdrr_project_staged_kernel<VW, SKEW><<<grid, kStageCtaThreads, smem, s>>>(p, map);
     return cudaGetLastError();
