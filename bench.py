@@ -95,6 +95,58 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def source_digest():
+    """sha256 over the CUDA sources: the stamp that ties profiles/ncu_constants.json to the kernels it was captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1204_6367_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            with open(os.path.join(csrc, name), "rb") as f:
+                h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()
+
+
+def ncu_constants(kernel, workload):
+    """Figures that only an `ncu --set full` capture can give (DRAM bytes, L2->SM bytes, the busy fraction of the bound),
+    from profiles/ncu_constants.json, written by hand from the committed capture summaries.  They are quoted only if the
+    capture was taken on the CUDA sources of this run (source_digest); else every figure is None."""
+    path = os.path.join(ROOT, "profiles", "ncu_constants.json")
+    none = {"dram_bytes_per_projection": None, "l2_to_sm_bytes_per_sample": None, "bound": "not profiled",
+            "bound_busy_frac": None, "capture": None, "matches_this_build": False}
+    if not os.path.exists(path):
+        return none
+    with open(path) as f:
+        table = json.load(f)
+    rec = table.get("kernels", {}).get(kernel, {}).get(workload)
+    if rec is None:
+        return none
+    rec = dict(rec)
+    rec["matches_this_build"] = table.get("source_sha256") == source_digest()
+    if not rec["matches_this_build"]:
+        for k in ("dram_bytes_per_projection", "l2_to_sm_bytes_per_sample", "bound_busy_frac"):
+            rec[k] = None
+        rec["bound"] = rec.get("bound", "") + " (capture is of older sources: figures withheld)"
+    return rec
+
+
+def cone_voxels(w, p):
+    """Voxels of the volume whose centre projects onto the detector at projection p: the least a projection must read."""
+    nx, ny, nz = w.dims
+    phi = float(w.phis[p])
+    c, s = np.cos(phi), np.sin(phi)
+    x = (np.arange(nx) - 0.5 * (nx - 1)) * w.spacing[0]
+    y = (np.arange(ny) - 0.5 * (ny - 1)) * w.spacing[1]
+    z = (np.arange(nz) - 0.5 * (nz - 1)) * w.spacing[2]
+    X, Y = np.meshgrid(x, y, indexing="xy")                       # [ny][nx]
+    depth = X * c + Y * s + w.sad                                  # along the central ray, from the source
+    u = (-X * s + Y * c) * w.sdd / depth - w.u_off
+    in_u = (np.abs(u) <= 0.5 * w.nu * w.du) & (depth > 0)
+    zmax = (0.5 * w.nv * w.dv + abs(w.v_off)) * depth / w.sdd     # |z| that still hits the detector, per (x, y)
+    per_column = (np.abs(z)[:, None, None] <= zmax[None]) & in_u[None]
+    return int(per_column.sum())
+
+
 def workload_config(w, name, world, n_total, launch_proj):
     nx, ny, nz = w.dims
     return {"workload": name, "volume": [nx, ny, nz], "voxel_mm": list(w.spacing),
@@ -156,7 +208,7 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     from workloads import make_workload
-    w = make_workload(args.workload)
+    w = make_workload(args.workload, phantom=args.phantom)
     pix, sample = sized_oracle_sample(w, args.ref_seconds)
     for _ in range(args.warmup):
         time_oracle(w, pix[: max(1, len(pix) // 16)])
@@ -188,7 +240,7 @@ def run_b200(args):
     import torch
     import paper_1204_6367_b200 as g
     from paper_1204_6367_b200 import dist as gd
-    from workloads import make_workload
+    from workloads import make_workload, pure_cell_fraction
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device; there is no CPU path")
@@ -200,7 +252,7 @@ def run_b200(args):
     peaks = measured_peaks()
 
     # the N-GPU job is one scan of n_proj * N evenly spaced angles, sharded by projection
-    w0 = make_workload(args.workload)
+    w0 = make_workload(args.workload, phantom=args.phantom)
     per_gpu = w0.n_proj if args.projections <= 0 else args.projections
     n_total = per_gpu * world
     mine = gd.strided_shard(n_total, world, rank)
@@ -319,45 +371,43 @@ def run_b200(args):
         return
 
     # ---- roofline of the dominant kernel (gdrr_project_kernel) ----------------------
+    picked = {g.GDRR_SAMPLER_STAGED: "gdrr_project_staged_kernel", g.GDRR_SAMPLER_GATHER: "gdrr_project_packed_kernel"}
     kname = ("gdrr_project_siddon_kernel" if args.method == "siddon" else
              "gdrr_project_texture_kernel" if args.method == "texture" else
              "gdrr_project_kernel" if args.layout != 2 else
-             "gdrr_project_packed_kernel" if args.sampler == "gather" else
-             "gdrr_project_staged_kernel" if args.sampler == "staged" else
-             "gdrr_project_staged_kernel (auto: gdrr_project_packed_kernel when a CTA's beam cannot fit the staged box)")
+             picked[g.gdrr_last_sampler(pr.ctx)])          # what --sampler auto launched (gdrr_last_sampler)
     corner_bytes = 4 if args.layout == 2 else 4 * vw        # packed word, or one float per material
     per_unit = 1 if args.method == "siddon" else 8          # one voxel per segment, 8 corners per sample
     l1_bytes = per_unit * corner_bytes * n_samples
     l1_peak = SM_COUNT * L1_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9       # GB/s
     l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
-    hbm_bytes = per_gpu * (vol_bytes + w.nu * w.nv * 4)
-    hbm_achieved = hbm_bytes / (kernel_ms * 1e-3) / 1e9
-    # dram__bytes_read + dram__bytes_write per launch, from the committed `ncu --set full` captures (8 projections of
-    # C3 per launch; per-projection figure x the projections of one launch here); other workloads: not captured
-    NCU_DRAM_PER_PROJECTION = {("C3", "gdrr_project_staged_kernel"): (3.392791e9 + 9.7344e6) / 8,      # profiles/r01_staged_kernel_ncu.md
-                               ("C3", "gdrr_project_packed_kernel"): (3.194201e9 + 10.405888e6) / 8,    # profiles/r01_packed_kernel_ncu.md
-                               ("C3", "gdrr_project_siddon_kernel"): (671.44704e6 + 9.620992e6) / 8}    # profiles/r01_siddon_kernel_ncu.md
-    ncu_traffic = args.ncu_dram_bytes if args.ncu_dram_bytes > 0 else None
-    if ncu_traffic is None and (args.workload, kname.split(" ")[0]) in NCU_DRAM_PER_PROJECTION:
-        ncu_traffic = NCU_DRAM_PER_PROJECTION[(args.workload, kname.split(" ")[0])] * launch_proj
+    # what only ncu can see comes from the committed capture of these very sources, or is None (never a stale constant)
+    ncu = ncu_constants(kname, args.workload if args.phantom == "smooth" and args.trajectory == "circle" else "-")
+    dram_step = ncu["dram_bytes_per_projection"] * per_gpu if ncu["dram_bytes_per_projection"] else None
+    # the least a projection must move: every voxel of its cone once as a 4-byte word, and its image
+    hbm_min = None
+    if w.poses is None:
+        probes = sorted({0, per_gpu // 8, per_gpu // 3})
+        hbm_min = float(np.mean([cone_voxels(w, p) for p in probes])) * 4.0 * per_gpu + per_gpu * w.nu * w.nv * 4.0
     roofline = {"kernel": kname, "bound": "l1tex", "achieved": l1_achieved, "peak": l1_peak,
-                "unit": "GB/s", "frac": l1_achieved / l1_peak, "traffic": ncu_traffic,
+                "unit": "GB/s", "frac": l1_achieved / l1_peak,
+                "traffic": dram_step / (-(-per_gpu // launch_proj)) if dram_step else None,
                 "kernel_ms_per_step": kernel_ms, "launches_per_step": -(-per_gpu // launch_proj),
                 "peak_def": f"{SM_COUNT} SMs x {L1_BYTES_PER_CLK} B/clk x {peaks['sm_max_mhz']:.0f} MHz (max SM clock)",
                 "algorithmic": f"{per_unit} voxel value(s) x {corner_bytes} B = {per_unit * corner_bytes} B per "
                                f"{'segment' if args.method == 'siddon' else 'sample'} through L1",
                 "samples_per_clk_per_sm": n_samples / (kernel_ms * 1e-3) / (SM_COUNT * peaks["sm_max_mhz"] * 1e6),
-                "ncu_identified_bound": {
-                    "gdrr_project_staged_kernel": "instruction issue: 77.6% of issue slots, L1 data pipe 63% (profiles/r01_staged_kernel_ncu.md)",
-                    "gdrr_project_packed_kernel": "L1 data-pipe wavefronts: 72% over a scan, 85-89% on one angle (profiles/r01_packed_kernel_ncu.md)",
-                    "gdrr_project_siddon_kernel": "instruction issue: 71% of issue slots, L1 20%; largest stall the wait for the next voxel (profiles/r01_siddon_kernel_ncu.md)",
-                }.get(kname.split(" ")[0], "not profiled"),
-                # busy fraction of that bound in the committed `ncu --set full` capture (8 projections of C3), not re-measured here
-                "ncu_bound_busy_frac": {"gdrr_project_staged_kernel": 0.776, "gdrr_project_packed_kernel": 0.715,
-                                        "gdrr_project_siddon_kernel": 0.709}.get(kname.split(" ")[0]),
-                "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                        "frac": hbm_achieved / peaks["hbm_gbs"], "peak_source": peaks["source"],
-                        "algorithmic": "device-layout volume once per projection + 4 B per pixel"}}
+                "ncu_identified_bound": ncu["bound"], "ncu_bound_busy_frac": ncu["bound_busy_frac"],
+                "ncu_capture": ncu["capture"], "ncu_capture_matches_this_build": ncu["matches_this_build"],
+                "l2_to_sm_bytes_per_sample": ncu["l2_to_sm_bytes_per_sample"],
+                # HBM: MEASURED dram bytes (the capture's per-projection figure x projections) over the live kernel time
+                "hbm": {"achieved": dram_step / (kernel_ms * 1e-3) / 1e9 if dram_step else None,
+                        "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": dram_step / (kernel_ms * 1e-3) / 1e9 / peaks["hbm_gbs"] if dram_step else None,
+                        "peak_source": peaks["source"],
+                        "dram_bytes_per_step": dram_step, "algorithmic_min_bytes_per_step": hbm_min,
+                        "traffic_vs_algorithmic": dram_step / hbm_min if dram_step and hbm_min else None,
+                        "algorithmic": "4 B per voxel of the projection's cone, once, + 4 B per pixel"}}
 
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload -----------
     cpu = None
@@ -366,15 +416,19 @@ def run_b200(args):
         n, dt, cores = time_oracle(w, pix)
         ref = time_oracle.last_signal
         got = signal.cpu().numpy()[pix[:, 0], pix[:, 2], pix[:, 1]].astype(np.float64)
+        pos = ref > 0.0                                     # (a zero oracle signal must be met exactly)
         cpu = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                "sample": f"{sample} ({n} samples)",
-               "max_rel_err_of_b200_signal_on_sample": float(np.max(np.abs(got - ref) / ref))}
+               "max_rel_err_of_b200_signal_on_sample": float(np.max(np.abs(got[pos] - ref[pos]) / ref[pos])) if pos.any() else 0.0,
+               "zero_signal_pixels_met_exactly": bool(np.all(got[~pos] == 0.0))}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "method": args.method, "sampler": args.sampler, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
             "config": dict(workload_config(w, args.workload, world, n_total, launch_proj),
+                           phantom=args.phantom, pure_cell_fraction=pure_cell_fraction(w.mat),
+                           inputs_sha256=w.sha256(),
                            **({} if args.trajectory == "circle" else {"trajectory": args.trajectory})),
             "projections_per_s": proj_per_s, "samples_per_step": total_samples,
             "paper_context": "paper: 1.2-2.3 s per poly-energetic projection on a GTX 580 (PAPER.md:366-367)",
@@ -479,13 +533,14 @@ def main():
                     help="source path: the paper's circle (the headline), a one-turn helix over half the volume's "
                          "height, or the circle tilted about x by --tilt-deg (gdrr_set_geometry_poses)")
     ap.add_argument("--tilt-deg", type=float, default=20.0)
+    ap.add_argument("--phantom", default="smooth", choices=["smooth", "noisy1", "noisy3", "random"],
+                    help="C2..C4: the BASELINE recipe (smooth), the same with 1 % / 3 % voxel noise before the material "
+                         "thresholds, or materials drawn per voxel (workloads/configs.py); the pure-cell fraction is printed")
     ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--ref-seconds", type=float, default=8.0, help="target oracle time per step of --impl reference")
-    ap.add_argument("--ncu-dram-bytes", type=float, default=0.0,
-                    help="dram bytes per launch from the committed ncu capture (profiles/)")
     args = ap.parse_args()
     global METRIC, UNIT
     if args.method == "denoise":

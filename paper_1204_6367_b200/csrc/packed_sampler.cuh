@@ -149,9 +149,8 @@ __device__ __forceinline__ void blend_general(const uint4& a, const uint4& c, fl
         route<VW>(A, c.z & 3u, fx * w01 * __uint_as_float(c.z));
         route<VW>(A, c.w & 3u, fx * w11 * __uint_as_float(c.w));
     }
-    // the running sum follows the material the ray is now in
-    const unsigned m4 = (c.w & 3u) | 4u;
-    if (m4 != A.curm4) switch_material<VW>(A, m4);
+    // (the running material changes only at a PURE cell of another material: following the corners of mixed cells makes
+    // it flip at every sample of a noisy volume, and every flip is a routed sum and a slow next sample)
 }
 
 // One sample.  UNI: every lane of the warp is here (unpredicated chunk): vote, so that the common case "all lanes

@@ -50,19 +50,28 @@ __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// (try_wait has acquire semantics, arrive has release semantics, both at CTA scope: the PTX defaults.  The last operand
-// is the time, in ns, the hardware may keep the warp suspended before try_wait returns false: long, so that a waiting
-// warp sleeps instead of spinning through issue slots)
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+// (try_wait has acquire semantics, arrive has release semantics, both at CTA scope: the PTX defaults)
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0u;
+}
+// A try_wait that fails returns after ~40 cycles (measured: the producer polled 88 times per wait), and a polling warp
+// takes issue slots from the sampling warps: sleep between polls.  SLEEP_NS = 0: poll.
+#ifndef GDRR_PRODUCER_SLEEP_NS
+#define GDRR_PRODUCER_SLEEP_NS 128
+#define GDRR_CONSUMER_SLEEP_NS 0
+#endif
+template <unsigned SLEEP_NS>
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    while (!mbar_try_wait(bar, parity)) {
+        if (SLEEP_NS) __nanosleep(SLEEP_NS);
+    }
 }
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
@@ -266,7 +275,7 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             const bool fit = mx[0] - mn[0] + 1 <= kBX && mx[1] - mn[1] + 1 <= kBY && mx[2] - mn[2] + 2 <= kBZ;
             skew_delay<SKEW>(8u + (unsigned)m, P.debug_skew);
             // stage st is free once every consumer warp has finished chunk m - 2
-            if (m >= 2) mbar_wait(bar_empty + 8u * st, (unsigned)((m >> 1) - 1) & 1u);
+            if (m >= 2) mbar_wait<GDRR_PRODUCER_SLEEP_NS>(bar_empty + 8u * st, (unsigned)((m >> 1) - 1) & 1u);
             if (lane == 0) {
                 ctl.fit[st] = fit;
                 // element of cell (cx, cy, cz) in the stage: lin + (cz kBY + cy) kBX + cx
@@ -316,7 +325,7 @@ gdrr_project_staged_kernel(const ProjectParams P, const __grid_constant__ CUtens
             const int bcx = W.cb[0], bcy = W.cb[1], bcz = W.cb[2];
             walk_advance(W);
             skew_delay<SKEW>((unsigned)(warp + 3 * m), P.debug_skew);
-            mbar_wait(bar_full + 8u * st, (unsigned)(m >> 1) & 1u);      // box landed (or: chunk does not fit); fit / lin valid
+            mbar_wait<GDRR_CONSUMER_SLEEP_NS>(bar_full + 8u * st, (unsigned)(m >> 1) & 1u);      // box landed (or: chunk does not fit); fit / lin valid
             const bool all_mine = m >= m_lo && m < m_hi;
             const int r = (c_begin + m) * kStageK - j0;         // the chunk's first index in this ray's own count
             const unsigned rel = (unsigned)r;

@@ -209,9 +209,18 @@ def _volume_c1(rng):
     return rho.astype(np.float32), mat, spacing, 2
 
 
-def _volume_pelvis(rng, dims, spacing):
+PHANTOMS = ("smooth", "noisy1", "noisy3", "random")
+
+
+def _volume_pelvis(rng, dims, spacing, phantom="smooth", seed=0):
     """Pelvis-like ellipsoid phantom, 4 materials by density thresholds
-    (used for C2, C3, C4 scaled to the extent)."""
+    (used for C2, C3, C4 scaled to the extent).
+
+    phantom: "smooth" (the recipe of BASELINE.md: noise-free densities, so 98.8 % of C3's cells have 8 corners of
+    one material); "noisy1" / "noisy3": the same densities times (1 + sigma z), z seeded unit Gaussian voxel
+    noise, sigma = 1 % / 3 %, applied to tissue BEFORE the thresholds, as in a reconstructed CT whose voxel noise
+    straddles the adipose / soft threshold; "random": the same densities with a material drawn uniformly per
+    voxel (no spatial structure at all: the worst case for any scheme that exploits material coherence)."""
     nx, ny, nz = dims
     shape = (nz, ny, nx)
     X, Y, Z = nx * spacing[0], ny * spacing[1], nz * spacing[2]
@@ -252,8 +261,34 @@ def _volume_pelvis(rng, dims, spacing):
     tex = _texture(shape, spacing)
     tissue = rho > np.float32(0.2)
     np.multiply(rho, tex, out=rho, where=tissue)
+    if phantom in ("noisy1", "noisy3"):
+        sigma = np.float32(0.01 if phantom == "noisy1" else 0.03)
+        gen = np.random.Generator(np.random.PCG64(seed))
+        for z in range(nz):                             # slab by slab: no second volume-sized array
+            noise = gen.standard_normal((ny, nx), dtype=np.float32)
+            np.multiply(rho[z], np.float32(1.0) + sigma * noise, out=rho[z], where=tissue[z])
+        np.maximum(rho, np.float32(0.0), out=rho)
     mat = _segment(rho)
+    if phantom == "random":
+        gen = np.random.Generator(np.random.PCG64(seed))
+        mat = gen.integers(0, 4, size=shape, dtype=np.uint8)
+    elif phantom not in PHANTOMS:
+        raise ValueError(f"unknown phantom {phantom!r}")
     return rho, mat, spacing, 4
+
+
+def pure_cell_fraction(mat):
+    """Fraction of the (nx-1)(ny-1)(nz-1) cells of the voxel lattice whose 8 corner voxels have one material
+    (an input statistic: the CUDA sampler's fast path needs such cells)."""
+    m = mat
+    same = np.ones(tuple(n - 1 for n in m.shape), dtype=bool)
+    ref = m[:-1, :-1, :-1]
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                if dz or dy or dx:
+                    same &= m[dz:m.shape[0] - 1 + dz, dy:m.shape[1] - 1 + dy, dx:m.shape[2] - 1 + dx] == ref
+    return float(same.mean())
 
 
 # --------------------------------------------------------------------------
@@ -282,11 +317,14 @@ def _even_angles(n):
 # public entry
 # --------------------------------------------------------------------------
 
-def make_workload(name: str, n_proj: Optional[int] = None) -> Workload:
+def make_workload(name: str, n_proj: Optional[int] = None, phantom: str = "smooth") -> Workload:
     """Build workload ``name`` in {"C0".."C4"}.  ``n_proj`` overrides the number
-    of evenly spaced projections (C3/C4 default to 360/656; C0..C2 to one at 0)."""
+    of evenly spaced projections (C3/C4 default to 360/656; C0..C2 to one at 0).
+    ``phantom`` (C2..C4 only): see _volume_pelvis; "smooth" is the configuration of BASELINE.json."""
     if name not in WORKLOAD_NAMES:
         raise ValueError(f"unknown workload {name!r}")
+    if phantom != "smooth" and name not in ("C2", "C3", "C4"):
+        raise ValueError("phantom variants exist for C2, C3 and C4")
     idx = WORKLOAD_NAMES.index(name)
     rng = SplitMix64(BASE_SEED + 1000 * idx)
     sad, sdd = 1000.0, 1500.0
@@ -314,7 +352,7 @@ def make_workload(name: str, n_proj: Optional[int] = None) -> Workload:
         else:
             dims, spacing = (512, 512, 512), (0.5, 0.5, 0.5)
             nu, nv, dpix, step, default_np = 1024, 768, 0.388, 0.25, 656
-        rho, mat, spacing, M = _volume_pelvis(rng, dims, spacing)
+        rho, mat, spacing, M = _volume_pelvis(rng, dims, spacing, phantom, BASE_SEED + 1000 * idx + 7)
         if name == "C4":
             E = 15.0 + (np.arange(120, dtype=np.float64) + 0.5) * 110.0 / 120.0
             e_max = 125.0
@@ -330,6 +368,7 @@ def make_workload(name: str, n_proj: Optional[int] = None) -> Workload:
     wl.rho = np.ascontiguousarray(wl.rho, dtype=np.float32)
     wl.mat = np.ascontiguousarray(wl.mat, dtype=np.uint8)
     wl.notes["seed"] = BASE_SEED + 1000 * idx
+    wl.notes["phantom"] = phantom
     return wl
 
 
