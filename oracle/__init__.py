@@ -41,7 +41,8 @@ def _load():
         _lib = ctypes.CDLL(_LIB)
         for name in ("gdrr_oracle_ray", "gdrr_oracle_trilinear", "gdrr_oracle_ray_samples",
                      "gdrr_oracle_project", "gdrr_oracle_project_siddon", "gdrr_oracle_project_literal",
-                     "gdrr_oracle_project_poses", "gdrr_oracle_ray_pose", "gdrr_oracle_denoise"):
+                     "gdrr_oracle_project_poses", "gdrr_oracle_ray_pose", "gdrr_oracle_denoise",
+                     "gdrr_oracle_project_general"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -162,6 +163,8 @@ def project(w, pixels=None, step=None, want_li=True, want_table=True, n_threads=
     """
     lib = _load()
     poses = getattr(w, "poses", None)
+    if getattr(w, "response_gain", None) is not None:
+        return _project_general(lib, w, pixels, step, want_li, want_table, n_threads, method)
     if poses is not None:
         return _project_poses(lib, w, _f64(poses).reshape(-1, 12), pixels, step, want_li, want_table,
                               n_threads, method)
@@ -192,6 +195,53 @@ def project(w, pixels=None, step=None, want_li=True, want_table=True, n_threads=
         raise ValueError(f"unknown method {method!r}")
     if rc:
         raise ValueError("gdrr_oracle_project: invalid arguments")
+    return out
+
+
+def _project_general(lib, w, pixels, step, want_li, want_table, n_threads, method):
+    """project() with a pixel-dependent detector response w.response_gain [n_energy][nv][nu] (reading Q32), on the
+    circular gantry or on w.poses: same outputs."""
+    if method not in ("trilinear", "siddon"):
+        raise ValueError(f"unknown method {method!r}")
+    rho = np.ascontiguousarray(w.rho, dtype=np.float32)
+    mat = np.ascontiguousarray(w.mat, dtype=np.uint8)
+    phi_w, resp, mu_hat = _f64(w.phi_weight), _f64(w.response), _f64(w.mu_hat)
+    flu = None if w.fluence_map is None else np.ascontiguousarray(w.fluence_map, dtype=np.float32)
+    bt_mu, bt_t = _f64(w.bowtie_mu), _f64(w.bowtie_thickness)
+    gain = np.ascontiguousarray(w.response_gain, dtype=np.float32)
+    if gain.shape != (phi_w.shape[0], w.nv, w.nu):
+        raise ValueError("response_gain must be [n_energy][nv][nu]")
+    poses = None if getattr(w, "poses", None) is None else _f64(w.poses).reshape(-1, 12)
+    phis = None if poses is not None else _f64(w.phis)
+    centre, ga = _geom_args(w)
+    M, n_proj = w.n_materials, (poses.shape[0] if poses is not None else phis.shape[0])
+    if pixels is None:
+        n_pix, pix = 0, None
+        signal = np.zeros((n_proj, w.nv, w.nu))
+        li = np.zeros((n_proj, M, w.nv, w.nu)) if want_li else None
+        tab = np.zeros((n_proj, w.nv, w.nu, 2), dtype=np.int32) if want_table else None
+    else:
+        pix = np.ascontiguousarray(pixels, dtype=np.int32).reshape(-1, 3)
+        n_pix = pix.shape[0]
+        signal = np.zeros(n_pix)
+        li = np.zeros((n_pix, M)) if want_li else None
+        tab = np.zeros((n_pix, 2), dtype=np.int32) if want_table else None
+    nseg = np.zeros(signal.shape, dtype=np.int32)
+    rc = lib.gdrr_oracle_project_general(
+        ctypes.c_int(1 if method == "siddon" else 0),
+        rho.ctypes.data_as(_c_float_p), mat.ctypes.data_as(_c_u8_p), *ga, ctypes.c_int(M), *_det_args(w),
+        ctypes.c_int(n_proj), _dp(phis), _dp(poses), ctypes.c_double(w.step_mm if step is None else step),
+        ctypes.c_int(phi_w.shape[0]), _dp(phi_w), _dp(resp), _dp(mu_hat),
+        None if flu is None else flu.ctypes.data_as(_c_float_p), _dp(bt_mu), _dp(bt_t),
+        gain.ctypes.data_as(_c_float_p),
+        ctypes.c_int64(n_pix), None if pix is None else pix.ctypes.data_as(_c_i32_p),
+        _dp(signal), _dp(li), None if tab is None else tab.ctypes.data_as(_c_i32_p),
+        nseg.ctypes.data_as(_c_i32_p), ctypes.c_int(n_threads))
+    if rc:
+        raise ValueError("gdrr_oracle_project_general: invalid arguments")
+    out = dict(signal=signal, line_integrals=li, ray_table=tab)
+    if method == "siddon":
+        out["n_segments"] = nseg
     return out
 
 

@@ -354,7 +354,9 @@ static int fill_setup(oracle_setup *g, const float *rho, const uint8_t *mat,
  * phi_b(E,u) = phi_E * w(u) * exp(-mu_bt(E) * t_bt(u)). */
 static double energy_sum(int n_energy, int n_materials, const double *phi_w,
                          const double *resp, const double *mu_hat, double w_pix,
-                         const double *bt_mu, double bt_t, const double *LI)
+                         const double *bt_mu, double bt_t, const double *LI,
+                         const float *gain_pix /* NULL, or this pixel's g(E, u) with stride gain_stride [Q32] */,
+                         size_t gain_stride)
 {
     double P = 0.0;
     for (int e = 0; e < n_energy; ++e) {
@@ -363,7 +365,10 @@ static double energy_sum(int n_energy, int n_materials, const double *phi_w,
             tau += mu_hat[(size_t)m * n_energy + e] * LI[m];
         double src = phi_w[e] * w_pix;
         if (bt_mu) src *= exp(-bt_mu[e] * bt_t);
-        P += src * resp[e] * exp(-tau);
+        /* r(E, u) = r(E) g(E, u): "In principle, the detector response could also be pixel dependent"
+         * (PAPER.md:111); g = 1 (NULL) is the paper's own pixel-independent case, bit for bit  [Q32] */
+        double r = gain_pix ? resp[e] * (double)gain_pix[(size_t)e * gain_stride] : resp[e];
+        P += src * r * exp(-tau);
     }
     return P;
 }
@@ -446,6 +451,7 @@ int gdrr_oracle_ray_samples(int nx, int ny, int nz, double dx, double dy, double
  */
 static int project_impl(int method /* 0 tri-linear midpoint rule, 1 Siddon */, int32_t *n_segments,
                         const double *poses /* [n_proj][12] or NULL = circular gantry */,
+                        const float *response_gain /* [n_energy][nv][nu] g(E, u) or NULL = 1  [Q32] */,
                         const float *rho, const uint8_t *mat,
                         int nx, int ny, int nz, double dx, double dy, double dz,
                         const double *centre, int n_materials,
@@ -501,7 +507,8 @@ static int project_impl(int method /* 0 tri-linear midpoint rule, 1 Siddon */, i
         }
         double w_pix = fluence ? (double)fluence[(size_t)j * nu + i] : 1.0;
         double bt_t = bt_thick ? bt_thick[i] : 0.0;
-        signal[q] = energy_sum(n_energy, M, phi_w, resp, mu_hat, w_pix, bt_mu, bt_t, LI);
+        signal[q] = energy_sum(n_energy, M, phi_w, resp, mu_hat, w_pix, bt_mu, bt_t, LI,
+                               response_gain ? response_gain + (size_t)j * nu + i : NULL, (size_t)nv * nu);
         if (line_integrals) {
             if (n_pix > 0) {
                 for (int m = 0; m < M; ++m) line_integrals[(size_t)q * M + m] = LI[m];
@@ -531,7 +538,7 @@ int gdrr_oracle_project(const float *rho, const uint8_t *mat,
                         double *signal, double *line_integrals, int32_t *ray_table,
                         int n_threads)
 {
-    return project_impl(0, NULL, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd, theta,
+    return project_impl(0, NULL, NULL, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd, theta,
                         nu, nv, du, dv, u_off, v_off, n_proj, phi, step, n_energy, phi_w, resp, mu_hat,
                         fluence, bt_mu, bt_thick, n_pix, pix, signal, line_integrals, ray_table, n_threads);
 }
@@ -551,7 +558,7 @@ int gdrr_oracle_project_siddon(const float *rho, const uint8_t *mat,
                         double *signal, double *line_integrals, int32_t *ray_table,
                         int32_t *n_segments, int n_threads)
 {
-    return project_impl(1, n_segments, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd,
+    return project_impl(1, n_segments, NULL, NULL, rho, mat, nx, ny, nz, dx, dy, dz, centre, n_materials, sad, sdd,
                         theta, nu, nv, du, dv, u_off, v_off, n_proj, phi, step, n_energy, phi_w, resp,
                         mu_hat, fluence, bt_mu, bt_thick, n_pix, pix, signal, line_integrals, ray_table,
                         n_threads);
@@ -574,9 +581,33 @@ int gdrr_oracle_project_poses(int method, const float *rho, const uint8_t *mat,
 {
     if (!poses || (method != 0 && method != 1)) return -1;
     /* sad, sdd are not used on this path: any valid pair passes fill_setup */
-    return project_impl(method, method == 1 ? n_segments : NULL, poses, rho, mat, nx, ny, nz, dx, dy, dz,
+    return project_impl(method, method == 1 ? n_segments : NULL, poses, NULL, rho, mat, nx, ny, nz, dx, dy, dz,
                         centre, n_materials, 1.0, 2.0, 0.0, nu, nv, du, dv, u_off, v_off, n_proj, NULL,
                         step, n_energy, phi_w, resp, mu_hat, fluence, bt_mu, bt_thick, n_pix, pix, signal,
+                        line_integrals, ray_table, n_threads);
+}
+
+/* The projector with every option: method 0 / 1, the circular gantry (phi, poses == NULL) or a general source path
+ * (poses, phi == NULL; sad, sdd, theta then unused), and a pixel-dependent detector response [Q32]
+ *   response_gain  [n_energy][nv][nu] float32 g(E, u), or NULL (= 1): r(E, u) = r(E) g(E, u). */
+int gdrr_oracle_project_general(int method, const float *rho, const uint8_t *mat,
+                        int nx, int ny, int nz, double dx, double dy, double dz,
+                        const double *centre, int n_materials,
+                        double sad, double sdd, double theta,
+                        int nu, int nv, double du, double dv, double u_off, double v_off,
+                        int n_proj, const double *phi, const double *poses, double step,
+                        int n_energy, const double *phi_w, const double *resp,
+                        const double *mu_hat, const float *fluence,
+                        const double *bt_mu, const double *bt_thick, const float *response_gain,
+                        int64_t n_pix, const int32_t *pix,
+                        double *signal, double *line_integrals, int32_t *ray_table,
+                        int32_t *n_segments, int n_threads)
+{
+    if ((method != 0 && method != 1) || ((phi == NULL) == (poses == NULL))) return -1;
+    if (poses) { sad = 1.0; sdd = 2.0; theta = 0.0; }
+    return project_impl(method, method == 1 ? n_segments : NULL, poses, response_gain, rho, mat, nx, ny, nz,
+                        dx, dy, dz, centre, n_materials, sad, sdd, theta, nu, nv, du, dv, u_off, v_off, n_proj,
+                        phi, step, n_energy, phi_w, resp, mu_hat, fluence, bt_mu, bt_thick, n_pix, pix, signal,
                         line_integrals, ray_table, n_threads);
 }
 

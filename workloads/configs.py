@@ -59,6 +59,9 @@ class Workload:
     # general source path (helical, C-arm): float64 [n_proj][12] = per projection source S, detector
     # origin P, u_hat, v_hat (world, mm); None = the circular gantry (sad, sdd, theta, phis)
     poses: Optional[np.ndarray] = None
+    # pixel-dependent detector response ("could also be pixel dependent"; reading Q32):
+    # float32 [n_energy][nv][nu] gain g(E, u), the pixel's response is response[E] * g; None = 1
+    response_gain: Optional[np.ndarray] = None
 
     @property
     def dims(self):
