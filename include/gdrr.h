@@ -122,27 +122,30 @@ GDRR_API const char* gdrr_last_error(const gdrr_context* ctx);
 GDRR_API int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int layout,
                                 size_t* bytes);
 
-/* Re-lays (rho, material) into the sampler's layout inside `workspace_dev`
- * with a CUDA kernel on `cuda_stream`, checks material < n_materials on the
- * device, and waits for that check (the only synchronising call besides the
- * *_host variants).
- *   rho_dev       [nz][ny][nx] fp32, x fastest, g/cm^3; borrowed for the call
- *   material_dev  [nz][ny][nx] uint8; borrowed for the call
+/* Re-lays (rho, material) into the sampler's layout inside `workspace_dev` with a CUDA kernel on `cuda_stream`
+ * and returns WITHOUT waiting for it: the volume can be used at once on any stream (the library orders its own
+ * kernels behind the ingest).  The ingest checks material < n_materials on the device; the verdict is read, never
+ * waited for, by every later call that takes the volume and finds the ingest finished, and by gdrr_volume_status,
+ * which waits.  A volume with a bad material index is refused from then on (INVALID_ARG); what was projected from
+ * it before is meaningless but in bounds.
+ *   rho_dev       [nz][ny][nx] fp32, x fastest, g/cm^3; borrowed until the ingest has run
+ *   material_dev  [nz][ny][nx] uint8; borrowed until the ingest has run
  *   d*_mm         voxel edge lengths; centre_mm = centre of the volume box in
  *                 world coordinates, NULL = the isocentre O
  *   workspace_dev >= gdrr_volume_workspace_bytes, 256-byte aligned, must
  *                 outlive the volume handle
- * Errors: INVALID_ARG (dims, spacings, NULLs, a material index out of range),
- * UNSUPPORTED (n_materials > GDRR_MAX_MATERIALS), WORKSPACE, CUDA. */
+ * Errors: INVALID_ARG (dims, spacings, NULLs), UNSUPPORTED (n_materials > GDRR_MAX_MATERIALS), WORKSPACE, CUDA. */
 GDRR_API int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* material_dev,
                        int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
                        const double centre_mm[3], int n_materials, int layout,
                        void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
                        gdrr_volume** out);
 
-/* Same, from HOST arrays: copies them into the caller's device staging buffers
- * (rho_stage_dev: nx*ny*nz floats, material_stage_dev: nx*ny*nz bytes) on the
- * stream, then proceeds as gdrr_create_volume. */
+/* Same, from HOST arrays (pinned for overlap): copies them into the caller's device staging buffers
+ * (rho_stage_dev: nx*ny*nz floats, material_stage_dev: nx*ny*nz bytes) in chunks of z slabs on a stream of the
+ * context, behind the work already queued on cuda_stream, and writes the slabs of the device layout that a chunk
+ * completes while the next chunk is on the bus.  Asynchronous like gdrr_create_volume; the host arrays must stay
+ * valid until cuda_stream has passed this point. */
 GDRR_API int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host,
                             const uint8_t* material_host,
                             int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
@@ -150,6 +153,10 @@ GDRR_API int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host,
                             float* rho_stage_dev, uint8_t* material_stage_dev,
                             void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
                             gdrr_volume** out);
+
+/* Waits for the volume's ingest and returns its verdict: OK, INVALID_ARG (a material index >= n_materials was met),
+ * CUDA.  The only call on a volume that blocks the host. */
+GDRR_API int gdrr_volume_status(gdrr_context* ctx, const gdrr_volume* vol);
 
 /* Frees the handle, never the workspace. */
 GDRR_API int gdrr_destroy_volume(gdrr_volume* vol);
@@ -194,6 +201,16 @@ GDRR_API int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,
                       const double* phi_weight, const double* response, const double* mu_hat,
                       const float* fluence_map, const double* bowtie_mu,
                       const double* bowtie_thickness_mm);
+
+/* Pixel-dependent detector response ("In principle, the detector response could also be pixel
+ * dependent.  In our calculation, we ignore this pixel dependence"; reading Q32):
+ *   gain [n_energy][nv][nu] fp32 g(E, u), host, copied to a context-owned device table (the library's one other
+ *        allocation of detector-sized memory besides the fluence map), or NULL to return to g = 1.
+ * The pixel's response becomes r(E, u) = response[E] * g(E, u) in every following gdrr_project; g = 1 gives the bits
+ * of the pixel-independent case.  Needs gdrr_set_geometry and gdrr_set_spectrum first (its shape) and is dropped
+ * when either changes the detector shape or the number of energy bins.
+ * Errors: NOT_READY, INVALID_ARG (a non-finite entry), CUDA. */
+GDRR_API int gdrr_set_response_gain(gdrr_context* ctx, const float* gain);
 
 /* ---- projection: steps a1-a7 -------------------------------------------- */
 

@@ -43,6 +43,7 @@ EXPORTS = (
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
     "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture", "gdrr_denoise_scatter",
     "gdrr_set_geometry_poses", "gdrr_last_sampler", "gdrr_debug_set_skew", "gdrr_debug_ray_cells",
+    "gdrr_set_response_gain", "gdrr_volume_status",
 )
 
 
@@ -68,6 +69,7 @@ def _load():
         "gdrr_create_volume": (i, [vp, vp, vp, i, i, i, d, d, d, vp, i, i, vp, sz, vp, pp]),
         "gdrr_create_volume_host": (i, [vp, vp, vp, i, i, i, d, d, d, vp, i, i, vp, vp, vp, sz, vp, pp]),
         "gdrr_destroy_volume": (i, [vp]),
+        "gdrr_volume_status": (i, [vp, vp]),
         "gdrr_set_geometry": (i, [vp, d, d, d, i, i, d, d, d, d, i, vp, d]),
         "gdrr_set_geometry_poses": (i, [vp, i, i, d, d, d, d, i, vp, d]),
         "gdrr_set_spectrum": (i, [vp, i, i, vp, vp, vp, vp, vp, vp]),
@@ -79,6 +81,7 @@ def _load():
         "gdrr_volume_attach_texture": (i, [vp, vp, vp]),
         "gdrr_denoise_scatter": (i, [vp, vp, vp, vp, i, i, i, d, d, i, d, vp]),
         "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
+        "gdrr_set_response_gain": (i, [vp, vp]),
         "gdrr_last_sampler": (i, [vp]),
         "gdrr_debug_set_skew": (i, [vp, i]),
         "gdrr_debug_ray_cells": (i, [vp, vp, i, i, i, i, vp, i, vp, vp]),
@@ -229,6 +232,11 @@ def _host_ptr(a, dtype_name, min_numel):
     raise TypeError("host buffer must be a numpy array or a CPU torch tensor")
 
 
+def gdrr_volume_status(ctx, vol):
+    """Waits for the volume's ingest; raises GdrrError(INVALID_ARG) if it met a material index >= n_materials."""
+    _check(_lib.gdrr_volume_status(ctx, vol), ctx)
+
+
 def gdrr_destroy_volume(vol):
     _check(_lib.gdrr_destroy_volume(vol))
 
@@ -270,6 +278,14 @@ def gdrr_set_spectrum(ctx, phi_weight, response, mu_hat, fluence_map=None, bowti
     _check(_lib.gdrr_set_spectrum(ctx, n_e, n_mat, pw_p, rs_p, mu_p, fl_p, bm_p, bt_p), ctx)
     if isinstance(ctx, _Context):
         ctx.n_mat = int(n_mat)
+
+
+def gdrr_set_response_gain(ctx, gain):
+    """gain: float32 [n_energy][nv][nu] (host) or None (= 1)."""
+    g, g_p = _host(gain, np.float32)
+    if g is not None and isinstance(ctx, _Context) and ctx.nu is not None and g.shape[1:] != (ctx.nv, ctx.nu):
+        raise ValueError("gain must be [n_energy][nv][nu]")
+    _check(_lib.gdrr_set_response_gain(ctx, g_p), ctx)
 
 
 def gdrr_project(ctx, vol, proj_begin, proj_count, signal_dev, line_integrals_dev=None,
@@ -371,6 +387,8 @@ class Projector:
                               w.phis, w.step_mm)
         gdrr_set_spectrum(self.ctx, w.phi_weight, w.response, w.mu_hat, w.fluence_map, w.bowtie_mu,
                           w.bowtie_thickness)
+        if getattr(w, "response_gain", None) is not None:
+            gdrr_set_response_gain(self.ctx, w.response_gain)
         nx, ny, nz = w.dims
         nbytes = gdrr_volume_workspace_bytes(nx, ny, nz, w.n_materials, layout)
         with torch.cuda.device(self.device):

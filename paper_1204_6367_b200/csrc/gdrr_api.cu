@@ -37,10 +37,18 @@ struct gdrr_context {
     float2* src_dev = nullptr;
     float* bt_dev = nullptr;
     float* flu_dev = nullptr;
+    float* gain_dev = nullptr;      // [n_energy][nv][nu] response gain (gdrr_set_response_gain) or nullptr
     // misc
-    int* flag_host = nullptr;       // pinned, mapped: the ingest kernel sets it through flag_dev if it meets a bad material
+    // pinned, mapped: an ingest kernel sets its volume's slot through flag_dev if it meets a bad material; the slots
+    // are handed out round-robin (a slot is reused after kFlagSlots later volumes)
+    static constexpr int kFlagSlots = 64;
+    int* flag_host = nullptr;
     int* flag_dev = nullptr;        //   (device address of flag_host)
+    unsigned next_flag = 0;
     cudaStream_t copy_stream = nullptr;
+    static constexpr int kIngestChunks = 8;             // gdrr_create_volume_host: z-slab chunks of the pipelined copy
+    cudaEvent_t ev_chunk[kIngestChunks] = {};
+    cudaEvent_t ev_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
     cudaEvent_t ev_free[2] = {nullptr, nullptr};
     int method = GDRR_METHOD_TRILINEAR;
@@ -63,6 +71,10 @@ struct gdrr_volume {
     bool compact_launched = false;
     cudaEvent_t compact_done = nullptr;
     bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
+    // the device-side material check is read when the ingest has finished, never waited for (volume_check)
+    cudaEvent_t ingest_done = nullptr;
+    volatile int* bad_flag = nullptr;    // this volume's slot of ctx->flag_host
+    bool checked = false, bad = false;
     cudaArray_t tex_array = nullptr;     // optional texture variant (gdrr_volume_attach_texture)
     cudaTextureObject_t tex = 0;
     alignas(64) CUtensorMap tmap;
@@ -169,12 +181,36 @@ int check_dims(gdrr_context* ctx, int nx, int ny, int nz, int n_materials, int l
     return GDRR_OK;
 }
 
+// The ingest kernels check material < n_materials on the device and raise the volume's flag (pinned host memory).
+// gdrr_create_volume does not wait for that: the flag is read here, by every later call that takes the volume, once the
+// ingest is known to have finished (cudaEventQuery; `wait`: cudaEventSynchronize, gdrr_volume_status).  A bad volume is
+// refused from then on.  (Its ingest wrote tags "material & 3", so nothing it did was out of bounds.)
+int volume_check(gdrr_context* ctx, const gdrr_volume* cvol, bool wait) {
+    gdrr_volume* vol = const_cast<gdrr_volume*>(cvol);
+    if (!vol->checked && vol->ingest_done) {
+        DeviceGuard guard(ctx->device);
+        cudaError_t e = wait ? cudaEventSynchronize(vol->ingest_done) : cudaEventQuery(vol->ingest_done);
+        if (e == cudaSuccess) {
+            vol->bad = *vol->bad_flag != 0;
+            vol->checked = true;
+        } else if (e != cudaErrorNotReady) {
+            return cuda_fail(ctx, e, "waiting for the volume ingest");
+        } else {
+            cudaGetLastError();
+        }
+    }
+    if (vol->bad)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "a material index of this volume is >= n_materials (%d)", vol->n_mat);
+    return GDRR_OK;
+}
+
 // Fills the fp64 ray-setup parameters for (ctx geometry, volume).  Box bounds
 // are formed exactly as DESIGN.md a1 writes them: half = 0.5 * (N * d).
 int fill_geom(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
               GeomParams& g) {
     if (!ctx->has_geom) return fail(ctx, GDRR_ERR_NOT_READY, "gdrr_set_geometry has not been called");
     if (!vol || vol->ctx != ctx) return fail(ctx, GDRR_ERR_INVALID_ARG, "volume is NULL or belongs to another context");
+    if (int rc = volume_check(ctx, vol, false)) return rc;
     if (proj_begin < 0 || proj_count <= 0 || proj_begin > ctx->n_proj - proj_count)
         return fail(ctx, GDRR_ERR_INVALID_ARG, "projection range [%d, %d+%d) outside [0, %d)", proj_begin,
                     proj_begin, proj_count, ctx->n_proj);
@@ -240,6 +276,7 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     P.src_tab = ctx->src_dev;
     P.bt_thick = ctx->bt_dev;
     P.fluence = ctx->flu_dev;
+    P.gain = ctx->gain_dev;
     P.n_energy = ctx->n_energy;
     P.n_mat = ctx->n_mat;
     // in-chunk positions are 9.23 fixed point: keep |advance| per chunk below 128 voxels
@@ -381,8 +418,16 @@ bool hull_margins(const gdrr_context* c, const gdrr_volume* vol, const GeomParam
     return ok;
 }
 
+// A kernel that reads the volume on stream s must run behind its ingest, whichever stream that was queued on
+// (gdrr_create_volume no longer waits for it).  Nothing to do once the ingest is known to have finished.
+cudaError_t order_after_ingest(const gdrr_volume* vol, cudaStream_t s) {
+    if (vol->checked || !vol->ingest_done) return cudaSuccess;
+    return cudaStreamWaitEvent(s, vol->ingest_done, 0);
+}
+
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
     gdrr_context* c = vol->ctx;
+    if (cudaError_t e = order_after_ingest(vol, s)) return e;
     if (c->method == GDRR_METHOD_SIDDON) {
         cudaError_t e = ensure_compact(vol, s);
         if (e != cudaSuccess) return e;
@@ -428,7 +473,7 @@ int gdrr_create_context(int cuda_device, gdrr_context** out) {
     ctx->device = cuda_device;
     DeviceGuard guard(cuda_device);
     if (guard.status != cudaSuccess) { delete ctx; return cuda_fail(nullptr, guard.status, "cudaSetDevice"); }
-    e = cudaHostAlloc(&ctx->flag_host, sizeof(int), cudaHostAllocMapped);
+    e = cudaHostAlloc(&ctx->flag_host, sizeof(int) * gdrr_context::kFlagSlots, cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->flag_dev, ctx->flag_host, 0);
     if (e != cudaSuccess) {
         if (ctx->flag_host) cudaFreeHost(ctx->flag_host);
@@ -443,12 +488,15 @@ int gdrr_destroy_context(gdrr_context* ctx) {
     if (!ctx) return GDRR_OK;
     DeviceGuard guard(ctx->device);
     free_dev(ctx->poses_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
-    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev);
+    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->gain_dev);
     if (ctx->flag_host) { cudaFreeHost(ctx->flag_host); ctx->flag_host = nullptr; ctx->flag_dev = nullptr; }
     for (int k = 0; k < 2; ++k) {
         if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
         if (ctx->ev_free[k]) cudaEventDestroy(ctx->ev_free[k]);
     }
+    for (int k = 0; k < gdrr_context::kIngestChunks; ++k)
+        if (ctx->ev_chunk[k]) cudaEventDestroy(ctx->ev_chunk[k]);
+    if (ctx->ev_stream) cudaEventDestroy(ctx->ev_stream);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     delete ctx;
     return GDRR_OK;
@@ -471,17 +519,14 @@ int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int lay
     return GDRR_OK;
 }
 
-int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* material_dev,
-                       int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
-                       const double centre_mm[3], int n_materials, int layout,
-                       void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
-                       gdrr_volume** out) {
-    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
-    if (!out) return fail(ctx, GDRR_ERR_INVALID_ARG, "out is NULL");
-    *out = nullptr;
-    int rc = check_dims(ctx, nx, ny, nz, n_materials, layout);
-    if (rc) return rc;
-    if (!rho_dev || !material_dev) return fail(ctx, GDRR_ERR_INVALID_ARG, "rho_dev / material_dev is NULL");
+// gdrr_create_volume and gdrr_create_volume_host.  rho_host / mat_host != NULL: the inputs are first copied into
+// rho_dev / mat_dev (the caller's staging buffers) in z-slab chunks on the context's copy stream, and the slabs of the
+// device layout that a chunk completes are written while the next chunk is still on the bus.
+static int create_volume_impl(gdrr_context* ctx, const float* rho_host, const uint8_t* mat_host,
+                              float* rho_dev, uint8_t* mat_dev, int nx, int ny, int nz,
+                              double dx_mm, double dy_mm, double dz_mm, const double centre_mm[3], int n_materials,
+                              int layout, void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                              gdrr_volume** out) {
     if (!(dx_mm > 0) || !(dy_mm > 0) || !(dz_mm > 0) || !std::isfinite(dx_mm) || !std::isfinite(dy_mm) ||
         !std::isfinite(dz_mm))
         return fail(ctx, GDRR_ERR_INVALID_ARG, "voxel sizes must be positive and finite");
@@ -496,13 +541,19 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    *ctx->flag_host = 0;            // (no kernel of this context is writing it: every ingest is waited for below)
-    cudaError_t e = cudaSuccess;
+    gdrr_volume* v = new (std::nothrow) gdrr_volume;
+    if (!v) return fail(ctx, GDRR_ERR_INVALID_ARG, "out of host memory");
+    cudaError_t e = cudaEventCreateWithFlags(&v->ingest_done, cudaEventDisableTiming);
+    if (e != cudaSuccess) { delete v; return cuda_fail(ctx, e, "cudaEventCreate"); }
+    const unsigned slot = ctx->next_flag++ % gdrr_context::kFlagSlots;
+    ctx->flag_host[slot] = 0;
+    v->bad_flag = ctx->flag_host + slot;
+
     IngestParams ip;
-    ip.rho = rho_dev; ip.mat = material_dev; ip.vox = workspace_dev;
+    ip.rho = rho_dev; ip.mat = mat_dev; ip.vox = workspace_dev;
     ip.nx = nx; ip.ny = ny; ip.nz = nz;
     stored_dims(nx, ny, nz, layout, ip.px, ip.py, ip.pz);
-    ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev;
+    ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev + slot;
     ip.sy = ip.sz = 0;
     ip.compact = nullptr; ip.cbx = (nx + 3) / 4; ip.cby = (ny + 3) / 4;
     if (layout == GDRR_LAYOUT_PACKED_QUAD) {
@@ -510,16 +561,50 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
         ip.compact = (char*)workspace_dev + ((16 * (size_t)ip.sz * ip.pz + 255) & ~(size_t)255);
     }
     const int vw = vector_width(n_materials);
-    e = launch_ingest(ip, vw, layout, s);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel launch");
-    ctx->launches += 1;
-    e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "ingest kernel");
-    const int bad = *(volatile int*)ctx->flag_host;
-    if (bad) return fail(ctx, GDRR_ERR_INVALID_ARG, "a material index is >= n_materials (%d)", n_materials);
-
-    gdrr_volume* v = new (std::nothrow) gdrr_volume;
-    if (!v) return fail(ctx, GDRR_ERR_INVALID_ARG, "out of host memory");
+    const size_t slab = (size_t)nx * ny;
+    // chunks of whole z slabs, at least ~4 MB of rho each; BRICK stores 2 x 2 x 2 bricks: one chunk
+    int chunks = 1;
+    if (rho_host && layout != GDRR_LAYOUT_BRICK)
+        chunks = (int)std::max<size_t>(1, std::min<size_t>({(size_t)gdrr_context::kIngestChunks, (size_t)nz,
+                                                             slab * nz * sizeof(float) / (4u << 20)}));
+    if (rho_host) {
+        if (!ctx->copy_stream) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+        for (int k = 0; k < gdrr_context::kIngestChunks && e == cudaSuccess; ++k)
+            if (!ctx->ev_chunk[k]) e = cudaEventCreateWithFlags(&ctx->ev_chunk[k], cudaEventDisableTiming);
+        if (e == cudaSuccess && !ctx->ev_stream) e = cudaEventCreateWithFlags(&ctx->ev_stream, cudaEventDisableTiming);
+        // the staging buffers may still be read by work queued on the caller's stream: the copies start behind it
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_stream, s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_stream, 0);
+    }
+    int stored_done = 0;                                   // stored slabs [0, stored_done) are written
+    for (int c = 0; c < chunks && e == cudaSuccess; ++c) {
+        const int z0 = (int)((long long)nz * c / chunks), z1 = (int)((long long)nz * (c + 1) / chunks);
+        if (rho_host) {
+            e = cudaMemcpyAsync(rho_dev + slab * z0, rho_host + slab * z0, slab * (z1 - z0) * sizeof(float),
+                                cudaMemcpyHostToDevice, ctx->copy_stream);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(mat_dev + slab * z0, mat_host + slab * z0, slab * (z1 - z0),
+                                    cudaMemcpyHostToDevice, ctx->copy_stream);
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_chunk[c], ctx->copy_stream);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ctx->ev_chunk[c], 0);
+        }
+        // stored slab k reads voxel slabs clamp(k - 1) (and clamp(k) for a quad's purity tags): with voxel slabs
+        // [0, z1) on the device, stored slabs up to z1 - 1 (quads), z1 (LINEAR) can be written; the last chunk the rest
+        int stored_end = c + 1 == chunks ? ip.pz : (layout == GDRR_LAYOUT_PACKED_QUAD ? z1 : z1 + 1);
+        if (stored_end > ip.pz) stored_end = ip.pz;
+        if (e == cudaSuccess && stored_end > stored_done) {
+            ip.ez0 = stored_done; ip.ezn = stored_end - stored_done;
+            e = launch_ingest(ip, vw, layout, s);
+            ctx->launches += 1;
+            stored_done = stored_end;
+        }
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(v->ingest_done, s);
+    if (e != cudaSuccess) {
+        cudaEventDestroy(v->ingest_done);
+        delete v;
+        return cuda_fail(ctx, e, "volume ingest");
+    }
     v->ctx = ctx; v->vox = workspace_dev;
     v->nx = nx; v->ny = ny; v->nz = nz; v->px = ip.px; v->py = ip.py; v->pz = ip.pz;
     v->d[0] = dx_mm; v->d[1] = dy_mm; v->d[2] = dz_mm;
@@ -529,6 +614,22 @@ int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* m
     v->has_tmap = layout == GDRR_LAYOUT_PACKED_QUAD && make_tensor_map(v);
     *out = v;
     return GDRR_OK;
+}
+
+int gdrr_create_volume(gdrr_context* ctx, const float* rho_dev, const uint8_t* material_dev,
+                       int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm,
+                       const double centre_mm[3], int n_materials, int layout,
+                       void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                       gdrr_volume** out) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!out) return fail(ctx, GDRR_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int rc = check_dims(ctx, nx, ny, nz, n_materials, layout);
+    if (rc) return rc;
+    if (!rho_dev || !material_dev) return fail(ctx, GDRR_ERR_INVALID_ARG, "rho_dev / material_dev is NULL");
+    return create_volume_impl(ctx, nullptr, nullptr, const_cast<float*>(rho_dev), const_cast<uint8_t*>(material_dev),
+                              nx, ny, nz, dx_mm, dy_mm, dz_mm, centre_mm, n_materials, layout, workspace_dev,
+                              workspace_bytes, cuda_stream, out);
 }
 
 int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host, const uint8_t* material_host,
@@ -544,21 +645,20 @@ int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host, const uint
     if (rc) return rc;
     if (!rho_host || !material_host || !rho_stage_dev || !material_stage_dev)
         return fail(ctx, GDRR_ERR_INVALID_ARG, "a host or staging pointer is NULL");
-    DeviceGuard guard(ctx->device);
-    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    const size_t nvox = (size_t)nx * ny * nz;
-    cudaError_t e = cudaMemcpyAsync(rho_stage_dev, rho_host, nvox * sizeof(float), cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess)
-        e = cudaMemcpyAsync(material_stage_dev, material_host, nvox, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "host-to-device copy of the volume");
-    return gdrr_create_volume(ctx, rho_stage_dev, material_stage_dev, nx, ny, nz, dx_mm, dy_mm, dz_mm,
-                              centre_mm, n_materials, layout, workspace_dev, workspace_bytes, cuda_stream, out);
+    return create_volume_impl(ctx, rho_host, material_host, rho_stage_dev, material_stage_dev, nx, ny, nz, dx_mm, dy_mm,
+                              dz_mm, centre_mm, n_materials, layout, workspace_dev, workspace_bytes, cuda_stream, out);
+}
+
+int gdrr_volume_status(gdrr_context* ctx, const gdrr_volume* vol) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!vol || vol->ctx != ctx) return fail(ctx, GDRR_ERR_INVALID_ARG, "volume is NULL or belongs to another context");
+    return volume_check(ctx, vol, true);
 }
 
 int gdrr_destroy_volume(gdrr_volume* vol) {
-    if (vol && (vol->tex || vol->tex_array || vol->compact_done)) {
+    if (vol && (vol->tex || vol->tex_array || vol->compact_done || vol->ingest_done)) {
         DeviceGuard guard(vol->ctx->device);
+        if (vol->ingest_done) cudaEventDestroy(vol->ingest_done);
         if (vol->tex) cudaDestroyTextureObject(vol->tex);
         if (vol->tex_array) cudaFreeArray(vol->tex_array);
         if (vol->compact_done) cudaEventDestroy(vol->compact_done);
@@ -579,7 +679,7 @@ static int install_geometry(gdrr_context* ctx, int nu, int nv, double du_mm, dou
     if (e != cudaSuccess) { cudaFree(dev); return cuda_fail(ctx, e, "cudaMemcpy(poses)"); }
     if (ctx->has_geom && (nu != ctx->nu || nv != ctx->nv)) {
         // tables shaped by the old detector are no longer valid
-        free_dev(ctx->flu_dev); free_dev(ctx->bt_dev);
+        free_dev(ctx->flu_dev); free_dev(ctx->bt_dev); free_dev(ctx->gain_dev);
         ctx->has_spec = false;
     }
     free_dev(ctx->poses_dev);
@@ -702,9 +802,29 @@ int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,
         return cuda_fail(ctx, e, "uploading the spectrum tables");
     }
     free_dev(ctx->mu_dev); free_dev(ctx->src_dev); free_dev(ctx->bt_dev); free_dev(ctx->flu_dev);
+    if (n_energy != ctx->n_energy) free_dev(ctx->gain_dev);        // shaped by the old energy grid
     ctx->mu_dev = mu_dev; ctx->src_dev = src_dev; ctx->bt_dev = bt_dev; ctx->flu_dev = flu_dev;
     ctx->n_energy = n_energy; ctx->n_mat = n_materials;
     ctx->has_spec = true;
+    return GDRR_OK;
+}
+
+int gdrr_set_response_gain(gdrr_context* ctx, const float* gain) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    if (!gain) { free_dev(ctx->gain_dev); return GDRR_OK; }
+    if (!ctx->has_geom || !ctx->has_spec)
+        return fail(ctx, GDRR_ERR_NOT_READY, "the response gain needs gdrr_set_geometry and gdrr_set_spectrum first (its shape)");
+    const size_t n = (size_t)ctx->n_energy * ctx->nv * ctx->nu;
+    for (size_t k = 0; k < n; ++k)
+        if (!std::isfinite(gain[k])) return fail(ctx, GDRR_ERR_INVALID_ARG, "a response gain entry is not finite");
+    float* dev = nullptr;
+    cudaError_t e = cudaMalloc(&dev, sizeof(float) * n);
+    if (e == cudaSuccess) e = cudaMemcpy(dev, gain, sizeof(float) * n, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { free_dev(dev); return cuda_fail(ctx, e, "uploading the response gain"); }
+    free_dev(ctx->gain_dev);
+    ctx->gain_dev = dev;
     return GDRR_OK;
 }
 
@@ -805,6 +925,8 @@ int gdrr_volume_attach_texture(gdrr_context* ctx, gdrr_volume* vol, void* cuda_s
     const cudaExtent ext = make_cudaExtent((size_t)vol->px, (size_t)vol->py, (size_t)vol->pz);
     cudaError_t e = cudaMalloc3DArray(&vol->tex_array, &desc, ext);
     if (e != cudaSuccess) { vol->tex_array = nullptr; return cuda_fail(ctx, e, "cudaMalloc3DArray"); }
+    e = order_after_ingest(vol, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamWaitEvent");
     cudaMemcpy3DParms cp = {};
     cp.srcPtr = make_cudaPitchedPtr(vol->vox, (size_t)vol->px * vw * sizeof(float), (size_t)vol->px, (size_t)vol->py);
     cp.dstArray = vol->tex_array;
@@ -869,7 +991,8 @@ int gdrr_siddon_segments(gdrr_context* ctx, const gdrr_volume* vol, int proj_beg
     P.signal = nullptr; P.li = nullptr; P.ray_table = nullptr; P.seg_table = n_segments_dev;
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
-    cudaError_t e = ensure_compact(vol, (cudaStream_t)cuda_stream);
+    cudaError_t e = order_after_ingest(vol, (cudaStream_t)cuda_stream);
+    if (e == cudaSuccess) e = ensure_compact(vol, (cudaStream_t)cuda_stream);
     if (e == cudaSuccess) e = launch_project_siddon(P, vol->vw, vol->layout, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "Siddon kernel launch");
     ctx->launches += 1;

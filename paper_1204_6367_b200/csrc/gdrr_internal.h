@@ -53,6 +53,7 @@ struct ProjectParams {
     const float2* src_tab;          // [n_energy] (phi_E * R_E, log2(e) * mu_bt[E])
     const float* bt_thick;          // [nu] or nullptr
     const float* fluence;           // [nv][nu] or nullptr
+    const float* gain;              // [n_energy][nv][nu] pixel-dependent response gain g(E, u) or nullptr (reading Q32)
     int n_energy, n_mat;
     int chunk;                      // <= kMaxChunk
     unsigned frac_mask, one_bits;   // 0x007FFFFF, 0x3F800000: kept in registers by the samplers
@@ -73,6 +74,7 @@ struct IngestParams {
     void* vox;
     int nx, ny, nz;
     int px, py, pz;                 // stored dims (voxels for BRICK / LINEAR, quads for PACKED_QUAD)
+    int ez0, ezn;                   // stored slabs [ez0, ez0 + ezn) to write in this launch (BRICK: always all of them)
     int sy, sz;                     // PACKED_QUAD: element strides (VolumeParams)
     void* compact;                  // PACKED_QUAD: the one-word-per-voxel copy, rows in groups of four
     int cbx, cby;                   //   ceil(nx / 4), ceil(ny / 4) (cby: groups of four rows per slab)

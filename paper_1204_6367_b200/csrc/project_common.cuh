@@ -74,10 +74,15 @@ __device__ __forceinline__ void finish_pixel(const ProjectParams& P, const float
             if (m < P.n_mat) o[m * plane] = li[m];
     }
     const float tb = P.bt_thick ? P.bt_thick[i] : 0.f;
+    // pixel-dependent detector response r(E, u) = r(E) g(E, u) (reading Q32): g streams in from global
+    // memory, energy-major, so that the pixels of a warp read neighbouring words
+    const size_t gain_plane = (size_t)P.g.nv * P.g.nu;
+    const float* gain = P.gain ? P.gain + (size_t)j * P.g.nu + i : nullptr;
     float sig = 0.f;
     for (int e = 0; e < P.n_energy; ++e) {
         const float4 mu = s_mu[e];
-        const float2 sc = s_src[e];
+        float2 sc = s_src[e];
+        if (gain) sc.x *= __ldg(gain + (size_t)e * gain_plane);
         float tau = sc.y * tb;
         tau = fmaf(mu.x, li[0], tau);
         if (VW > 1) tau = fmaf(mu.y, li[VW > 1 ? 1 : 0], tau);

@@ -16,7 +16,7 @@
 // a PACKED_QUAD volume carries a second, compact copy for this walk: the same tagged word per
 // voxel, rows in groups of four (4 B per voxel instead of 16; a 128-byte line is 8 x 4 voxels).
 // fp32 accumulation is chunked like the tri-linear sampler's (32 segments per partial sum).
-#include "project_common.cuh"
+#include "packed_sampler.cuh"
 
 namespace gdrr {
 
@@ -37,12 +37,6 @@ __device__ __forceinline__ void add_len(float (&a)[4], float len, const float4& 
     a[3] = fmaf(len, v.w, a[3]);
 }
 
-template <int VW>
-__device__ __forceinline__ void add_routed_s(float (&part)[VW], int m, float v) {
-#pragma unroll
-    for (int k = 0; k < VW; ++k) part[k] += (m == k) ? v : 0.f;
-}
-
 // Element offset contributed by voxel index i along one axis.  LAYOUT 0: padded 2x2x2 bricks of the exact
 // BRICK layout (project_fused.cu has the same map); 1: padded linear; 2: the packed volume's compact copy,
 // unpadded, rows in groups of four: iz SZ + (iy >> 2) SY + 4 ix + (iy & 3) (volume_layout.cu).
@@ -55,24 +49,9 @@ __device__ __forceinline__ int siddon_axis_offset(int i, int stride) {
     return i * stride;
 }
 
-// len x voxel value into the per-material sums.  Exact layouts: one FMA per material.  Packed word:
-// a running sum of the current material, routed when the material changes.
-template <int VW, int LAYOUT, class VT>
-__device__ __forceinline__ void accumulate_voxel(const VT& v, float len, float (&part)[VW], float& cur, unsigned& curm) {
-    if constexpr (LAYOUT == 2) {
-        if (VW > 1) {
-            const unsigned m = v & 3u;
-            if (m != curm) {
-                add_routed_s<VW>(part, (int)curm, cur);
-                cur = 0.f;
-                curm = m;
-            }
-        }
-        cur = fmaf(len, __uint_as_float(v), cur);
-    } else {
-        add_len(part, len, v);
-    }
-}
+// The material of the walk changes (a few times per ray): the closed run goes to its material's slot.  Out of line, so
+// that the walk's loop keeps a plain branch around it instead of ten predicated instructions in every step.
+__device__ __noinline__ void route_out_of_line(float* slot, unsigned m, float v) { slot[m * kAccStride] += v; }
 
 // One voxel value: the exact layouts hold VW floats, the packed layout one tagged word.
 template <int VW, int LAYOUT> struct SiddonVoxel { using T = typename SVox<VW>::T; };
@@ -90,6 +69,7 @@ template <int VW, int LAYOUT, bool COUNT>
 __global__ void __launch_bounds__(kThreads)
 gdrr_project_siddon_kernel(const ProjectParams P) {
     using VT = typename SiddonVoxel<VW, LAYOUT>::T;
+    __shared__ float s_acc[LAYOUT == 2 ? 4 : 1][LAYOUT == 2 ? kAccStride : 1];      // per-material sums of a packed walk
     float4* s_mu;
     float2* s_src;
     load_tables(P, s_mu, s_src);
@@ -147,64 +127,83 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
         // linear element orders: stepping one voxel along an axis adds a constant to the element offset
         const int dox = stp[0] * (LAYOUT == 2 ? 4 : sx), doy = stp[1] * sy, doz = stp[2] * sz;
         const int y_edge = stp[1] > 0 ? 3 : 0, doy_cross = stp[1] * (sy - 3);       // LAYOUT 2 only
-        float kx = 0.f, ky = 0.f, kz = 0.f;              // planes crossed so far per axis (exact in fp32)
+        // 1 / dt for the re-base (0 for an axis the ray does not move along: its parameter stays 3e38)
+        const float idt[3] = {dt[0] > 0.f ? 1.f / dt[0] : 0.f, dt[1] > 0.f ? 1.f / dt[1] : 0.f,
+                              dt[2] > 0.f ? 1.f / dt[2] : 0.f};
         float tx = t0[0], ty = t0[1], tz = t0[2];
         float t = 0.f;
-        unsigned curm = 0;
-        float cur = 0.f;
+        RayAcc<VW> A;                                    // LAYOUT 2: running sum of the current material (packed_sampler.cuh)
+        if (LAYOUT == 2) init_ray<VW>(A, &s_acc[0][threadIdx.x]);
 
-        // the voxel of segment s + 1 is requested before segment s is accumulated
-        VT v = load_voxel<VW, LAYOUT>(vox, off);
+        // the walk moves a pointer; the voxel of segment s + 1 is requested before segment s is accumulated.
+        // (compact copy: its base is 256-byte aligned and SY, SZ are multiples of 4 words, so bits 2-3 of the
+        // address are the row's place in its group of four)
+        const VT* ptr = reinterpret_cast<const VT*>(vox) + off;
+        const unsigned y_edge_bits = 4u * (unsigned)y_edge;
+        VT v = __ldg(ptr);
         bool more = true;
         while (more) {
             float part[VW];
 #pragma unroll
             for (int m = 0; m < VW; ++m) part[m] = 0.f;
+            // Inside a chunk the crossed axis' parameter moves by one addition.  At a chunk's start the three are formed
+            // anew from the number of planes crossed, which the drifted value still gives exactly when rounded
+            // (drift <= 16 ulp of the chord, dt >= a voxel edge).
+            tx = fmaf(rintf((tx - t0[0]) * idt[0]), dt[0], t0[0]);
+            ty = fmaf(rintf((ty - t0[1]) * idt[1]), dt[1], t0[1]);
+            tz = fmaf(rintf((tz - t0[2]) * idt[2]), dt[2], t0[2]);
+#pragma unroll 2
             for (int s = 0; s < kMaxChunk && more; ++s) {
                 const float tn = fminf(fminf(tx, ty), fminf(tz, t_end));    // where the ray leaves this voxel
-                const float len = tn - t;
-                t = fmaxf(tn, t);
+                const float tnew = fmaxf(tn, t);
+                const float len = tnew - t;                                 // >= 0
+                t = tnew;
                 more = tn < t_stop;
-                // cross the plane that was met (x before y before z at ties), branch-free
-                const bool bx = tx <= ty && tx <= tz;
-                const bool by = !bx && ty <= tz;
+                // cross the plane that was met (x before y before z at ties)
+                const bool bx = tx == tn;
+                const bool by = !bx && ty == tn;
                 if (LAYOUT == 0) {
                     idx[0] += bx ? stp[0] : 0;
                     idx[1] += by ? stp[1] : 0;
                     idx[2] += (bx || by) ? 0 : stp[2];
-                    // (past the last voxel the walk has stepped out of the lattice: keep the last valid offset)
-                    const int o = siddon_axis_offset<LAYOUT, 0>(idx[0], sx) + siddon_axis_offset<LAYOUT, 1>(idx[1], sy) +
-                                  siddon_axis_offset<LAYOUT, 2>(idx[2], sz);
-                    off = more ? o : off;
+                    ptr = reinterpret_cast<const VT*>(vox) + (siddon_axis_offset<LAYOUT, 0>(idx[0], sx) +
+                          siddon_axis_offset<LAYOUT, 1>(idx[1], sy) + siddon_axis_offset<LAYOUT, 2>(idx[2], sz));
                 } else if (LAYOUT == 2) {
                     // rows in groups of 4: a step in y moves by one word inside a group, by a row of groups across its edge
-                    const int dy_now = ((idx[1] & 3) == y_edge) ? doy_cross : stp[1];
-                    idx[1] += by ? stp[1] : 0;
-                    off += more ? (bx ? dox : (by ? dy_now : doz)) : 0;
+                    const int dy_now = (((unsigned)(uintptr_t)ptr & 12u) == y_edge_bits) ? doy_cross : stp[1];
+                    ptr += bx ? dox : (by ? dy_now : doz);
                 } else {
-                    off += more ? (bx ? dox : (by ? doy : doz)) : 0;
+                    ptr += bx ? dox : (by ? doy : doz);
                 }
-                // plane counters and parameters of all three axes, without branches (only one counter moves)
-                kx += bx ? 1.f : 0.f;
-                ky += by ? 1.f : 0.f;
-                kz += (bx || by) ? 0.f : 1.f;
-                tx = fmaf(kx, dt[0], t0[0]);
-                ty = fmaf(ky, dt[1], t0[1]);
-                tz = fmaf(kz, dt[2], t0[2]);
+                if (bx) tx += dt[0];
+                if (by) ty += dt[1];
+                if (!bx && !by) tz += dt[2];
                 const VT cv = v;
-                v = load_voxel<VW, LAYOUT>(vox, off);          // when the walk is over: the last voxel again, unused
-                if (len > 0.f) {
-                    if (COUNT) ++n_seg;
-                    accumulate_voxel<VW, LAYOUT>(cv, len, part, cur, curm);
+                if (more) v = __ldg(ptr);                                   // (past the end the walk has left the lattice)
+                if (COUNT) n_seg += len > 0.f ? 1 : 0;
+                if constexpr (LAYOUT == 2) {
+                    if (VW > 1) {
+                        const unsigned m4 = (cv & 3u) | 4u;
+                        if (m4 != A.curm4) {
+                            route_out_of_line(A.slot, A.curm4 & 3u, A.cur + A.run);
+                            A.cur = 0.f;
+                            A.run = 0.f;
+                            A.curm4 = m4;
+                        }
+                    }
+                    A.cur = fmaf(len, __uint_as_float(cv), A.cur);
+                } else {
+                    add_len(part, len, cv);
                 }
             }
             if (LAYOUT == 2) {
-                add_routed_s<VW>(part, (int)curm, cur);
-                cur = 0.f;
-            }
+                flush_chunk<VW>(A);
+            } else {
 #pragma unroll
-            for (int m = 0; m < VW; ++m) acc[m] += part[m];
+                for (int m = 0; m < VW; ++m) acc[m] += part[m];
+            }
         }
+        if (LAYOUT == 2) finish_ray<VW>(A, acc);
     }
 
     if (COUNT && P.seg_table) P.seg_table[pix] = n_seg;

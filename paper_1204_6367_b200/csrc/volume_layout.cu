@@ -29,8 +29,9 @@ template <int VW, int LAYOUT>
 __global__ void __launch_bounds__(256)
 gdrr_ingest_kernel(const IngestParams P) {
     using V = typename VoxT<VW>::T;
-    const size_t total = (size_t)P.px * P.py * P.pz;
-    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // stored slabs [ez0, ez0 + ezn) of the padded volume (LINEAR), or everything (BRICK: ez0 = 0, ezn = pz)
+    const size_t first = (size_t)P.px * P.py * P.ez0, total = (size_t)P.px * P.py * (P.ez0 + P.ezn);
+    const size_t o = first + (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= total) return;
     int sx_, sy_, sz_;      // stored (padded) coordinates of element o
     if (LAYOUT == 0) {
@@ -75,7 +76,7 @@ gdrr_ingest_kernel(const IngestParams P) {
 // y = row, z = slab: no division in the index arithmetic.
 __global__ void __launch_bounds__(256)
 gdrr_ingest_packed_kernel(const IngestParams P) {
-    const int ez = blockIdx.z, ey = blockIdx.y;
+    const int ez = P.ez0 + blockIdx.z, ey = blockIdx.y;
     int ex = blockIdx.x * blockDim.x + threadIdx.x;
     const int row_slots = (ey == P.py - 1) ? P.sz - ey * P.sy : P.sy;      // the last row also owns the slab's tail pad
     if (ex >= row_slots) return;
@@ -141,7 +142,7 @@ gdrr_ingest_compact_kernel(const IngestParams P) {
 
 template <int VW, int LAYOUT>
 static cudaError_t launch_ingest_t(const IngestParams& p, cudaStream_t s) {
-    const size_t total = (size_t)p.px * p.py * p.pz;
+    const size_t total = (size_t)p.px * p.py * p.ezn;
     const unsigned int blocks = (unsigned int)((total + 255) / 256);
     gdrr_ingest_kernel<VW, LAYOUT><<<blocks, 256, 0, s>>>(p);
     return cudaGetLastError();
@@ -156,7 +157,7 @@ cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_
     if (layout == 2) {
         // (py and pz, cby and nz stay far below the 65535 limit of grid.y / grid.z for any volume that fits int32 indexing)
         const int row_max = p.sy + 8;                                   // a row, or the last row plus the slab's tail pad
-        gdrr_ingest_packed_kernel<<<dim3((row_max + 255) / 256, p.py, p.pz), 256, 0, s>>>(p);
+        gdrr_ingest_packed_kernel<<<dim3((row_max + 255) / 256, p.py, p.ezn), 256, 0, s>>>(p);
         return cudaGetLastError();
     }
     if (layout == 0) {

@@ -320,14 +320,33 @@ def test_error_codes_on_device(gdrr):
             gdrr.gdrr_project(ctx, vol, 0, 2, sig)                  # an output tensor smaller than the request
         gdrr.gdrr_project(ctx, vol, 0, 1, sig)
         torch.cuda.synchronize()
-        # a material index out of range is caught on the device
-        mat[1, 2, 3] = 5
+        # a material index out of range is caught on the device: gdrr_create_volume does not wait for the check,
+        # gdrr_volume_status does, and every later call on the volume refuses it
+        gdrr.gdrr_volume_status(ctx, vol)                       # the good volume
+        mat_bad = mat.clone()
+        mat_bad[1, 2, 3] = 5
+        ws2 = torch.empty_like(ws)
+        bad = gdrr.gdrr_create_volume(ctx, rho, mat_bad, (4, 4, 4), (1, 1, 1), None, 1, 0, ws2)
         with pytest.raises(gdrr.GdrrError) as e:
-            gdrr.gdrr_create_volume(ctx, rho, mat, (4, 4, 4), (1, 1, 1), None, 1, 0, ws)
+            gdrr.gdrr_volume_status(ctx, bad)
         assert e.value.code == gdrr.GDRR_ERR_INVALID_ARG
+        with pytest.raises(gdrr.GdrrError) as e:
+            gdrr.gdrr_project(ctx, bad, 0, 1, sig)
+        assert e.value.code == gdrr.GDRR_ERR_INVALID_ARG
+        gdrr.gdrr_destroy_volume(bad)
+        # ... also without gdrr_volume_status, by the first call that finds the ingest finished
+        for layout in (0, 1, 2):
+            wsl = torch.empty(gdrr.gdrr_volume_workspace_bytes(4, 4, 4, 1, layout), dtype=torch.uint8, device="cuda")
+            bad = gdrr.gdrr_create_volume(ctx, rho, mat_bad, (4, 4, 4), (1, 1, 1), None, 1, layout, wsl)
+            torch.cuda.synchronize()
+            with pytest.raises(gdrr.GdrrError) as e:
+                gdrr.gdrr_project(ctx, bad, 0, 1, sig)
+            assert e.value.code == gdrr.GDRR_ERR_INVALID_ARG
+            gdrr.gdrr_destroy_volume(bad)
+        gdrr.gdrr_project(ctx, vol, 0, 1, sig)                  # the good volume still works
         # workspace too small
         with pytest.raises(gdrr.GdrrError) as e:
-            gdrr.gdrr_create_volume(ctx, rho, mat * 0, (4, 4, 4), (1, 1, 1), None, 1, 0, ws[:100])
+            gdrr.gdrr_create_volume(ctx, rho, mat, (4, 4, 4), (1, 1, 1), None, 1, 0, ws[:100])
         assert e.value.code == gdrr.GDRR_ERR_WORKSPACE
         # source inside the volume box
         big = tiny_workload(np.ones((4, 4, 4), dtype=np.float32), spacing=(600.0, 600.0, 600.0))
