@@ -857,14 +857,12 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSuccess;
-    if (!ctx->copy_stream) {
-        e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
-        for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
-            e = cudaEventCreateWithFlags(&ctx->ev_done[k], cudaEventDisableTiming);
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_free[k], cudaEventDisableTiming);
-        }
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "creating the copy stream");
+    if (!ctx->copy_stream) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+        if (!ctx->ev_done[k]) e = cudaEventCreateWithFlags(&ctx->ev_done[k], cudaEventDisableTiming);
+        if (e == cudaSuccess && !ctx->ev_free[k]) e = cudaEventCreateWithFlags(&ctx->ev_free[k], cudaEventDisableTiming);
     }
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "creating the copy stream");
     // two half-buffers: the kernel fills one while the other drains to the host
     const size_t plane = (size_t)ctx->nu * ctx->nv;
     const int slots = stage_proj >= 2 ? 2 : 1;

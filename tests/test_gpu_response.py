@@ -69,12 +69,13 @@ def test_unit_gain_and_clearing_give_the_plain_bits(gdrr, workloads_cache):
 
 
 def test_half_fan_detector_offset(gdrr, workloads_cache):
-    """A half-fan scan: the detector shifted by 148 mm, so that most rays of one side miss the volume's far half and
-    many cross it only partly; per-pixel parity on two full C2-sized projections."""
+    """A half-fan scan: the detector shifted by 148 mm, so that the rays of its far edge cross only a corner of the
+    volume; per-pixel parity on two full C2-sized projections."""
     w = copy.copy(workloads_cache("C2").with_phis(np.radians([0.0, 123.0])))
     w.u_off = 148.0
     ref = oracle.project(w)
     with gdrr.Projector(w) as pr:
         stats = compare_full(pr, w, ref, "half fan")
-    assert (ref["ray_table"][..., 1] == 0).mean() > 0.02          # a visible share of the rays misses
+    n = ref["ray_table"][..., 1]
+    assert n.min() < 0.5 * n.max()                                # chords from a corner of the box to its full width
     print(stats)

@@ -6,9 +6,10 @@ floor, exactly 0 where the oracle has 0, the midpoint ray table (a property of t
 the method) bit-exact.  The number of voxel segments of positive length is unique only in exact
 arithmetic: where a ray passes within rounding of a lattice edge (near-ties, frequent for rays that
 run almost inside a lattice plane of these symmetric phantoms) a sliver of 1e-6 mm exists in fp64
-and not in fp32.  So the hit mask must be identical, and the counts must agree on all but a few
-percent of the rays, within a few percent per ray, and in total to 1e-3 (measured on C2: 0.5% of
-the rays differ, by at most 10 of ~280 segments)."""
+and not in fp32.  So the hit mask must be identical, the counts must agree on all but 1 % of the
+rays (3 % for C1 seen along a lattice axis) within 10 segments per ray, and in total to 1e-3
+(measured in round 2: 0.43 % of C2's rays at 0 and 90 degrees differ, by at most 8 of ~280 segments; 0.02 % by at
+most 1 at 37 and 225 degrees; 2.6 % by at most 3 on C1 at 0 degrees)."""
 import math
 
 import numpy as np
@@ -31,17 +32,18 @@ def gdrr():
     return g
 
 
-def check_segments(seg_gpu, seg_ref, what=""):
+def check_segments(seg_gpu, seg_ref, what="", max_fraction=0.01):
     seg_gpu, seg_ref = np.asarray(seg_gpu, dtype=np.int64), np.asarray(seg_ref, dtype=np.int64)
     assert seg_gpu.shape == seg_ref.shape
     assert np.array_equal(seg_gpu == 0, seg_ref == 0), f"{what}: hit mask differs"
     diff = np.abs(seg_gpu - seg_ref)
-    assert np.all(diff <= 4 + 0.05 * seg_ref), f"{what}: segment counts differ by up to {int(diff.max())}"
-    assert np.count_nonzero(diff) <= max(3, 0.03 * diff.size), f"{what}: {np.count_nonzero(diff)} rays differ"
+    print(f"{what}: segment counts differ on {np.count_nonzero(diff)} of {diff.size} rays, by at most {int(diff.max())}")
+    assert np.all(diff <= 10), f"{what}: segment counts differ by up to {int(diff.max())}"
+    assert np.count_nonzero(diff) <= max(3, max_fraction * diff.size), f"{what}: {np.count_nonzero(diff)} rays differ"
     assert abs(int(seg_gpu.sum()) - int(seg_ref.sum())) <= max(3, 1e-3 * int(seg_ref.sum())), what
 
 
-def compare_full_siddon(g, w, layout, what):
+def compare_full_siddon(g, w, layout, what, max_fraction=0.01):
     ref = oracle.project(w, method="siddon")
     with g.Projector(w, layout=layout, method=g.GDRR_METHOD_SIDDON) as pr:
         sig, li, tab = pr.project(want_li=True, want_table=True)
@@ -49,7 +51,7 @@ def compare_full_siddon(g, w, layout, what):
     check_ray_table(tab.cpu().numpy(), ref["ray_table"], what)
     rel_li, n_floor = check_line_integrals(li.cpu().numpy(), ref["line_integrals"], what)
     worst = check_signal(sig.cpu().numpy(), ref["signal"], what)
-    check_segments(seg.cpu().numpy(), ref["n_segments"], what)
+    check_segments(seg.cpu().numpy(), ref["n_segments"], what, max_fraction)
     print(what, "signal", worst, "LI", rel_li, "floor pixels", n_floor)
     return ref
 
@@ -57,7 +59,9 @@ def compare_full_siddon(g, w, layout, what):
 @pytest.mark.parametrize("layout", [0, 1, 2])
 @pytest.mark.parametrize("name", ["C0", "C1"])
 def test_siddon_full_image_small(gdrr, workloads_cache, name, layout):
-    compare_full_siddon(gdrr, workloads_cache(name), layout, f"siddon {name} layout {layout}")
+    # (C1 at phi = 0: a symmetric phantom seen along a lattice axis, 2.6 % of its rays run within rounding of a lattice
+    # plane; the envelope everywhere else is 1 % of the rays)
+    compare_full_siddon(gdrr, workloads_cache(name), layout, f"siddon {name} layout {layout}", max_fraction=0.03)
 
 
 @pytest.mark.parametrize("phi_deg", [0.0, 37.0, 90.0, 225.0])
