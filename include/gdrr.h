@@ -102,7 +102,12 @@ enum {
                                   does not fit is gathered; GATHER is used if 16 steps exceed 15 voxels) */
 };
 
-#define GDRR_MAX_MATERIALS 4
+/* Up to four materials a volume is ONE device volume and gdrr_project one kernel.  More (PAPER.md:97 puts no bound on
+ * the material index): the volume is kept as ceil(n / 4) device volumes, one per group of four materials, in each of
+ * which the voxels of the other groups are empty; gdrr_project then samples every group (one launch each, writing that
+ * group's line integrals) and forms the signal from all line integrals in one more kernel.  Time and workspace grow
+ * with the number of groups. */
+#define GDRR_MAX_MATERIALS 16
 #define GDRR_MAX_ENERGIES 512
 
 /* ---- context ----------------------------------------------------------- */
@@ -218,7 +223,8 @@ GDRR_API int gdrr_set_response_gain(gdrr_context* ctx, const float* gain);
  * asynchronously on `cuda_stream`; outputs are valid once the stream reaches
  * this point.
  *   signal_dev         out [proj_count][nv][nu] fp32, required
- *   line_integrals_dev out [proj_count][n_materials][nv][nu] fp32, or NULL
+ *   line_integrals_dev out [proj_count][n_materials][nv][nu] fp32, or NULL (REQUIRED with more than four materials:
+ *                      the groups' line integrals wait there for the energy sum)
  *   ray_table_dev      out [proj_count][nv][nu][2] int32 = (j0, n): index of the
  *                      first midpoint inside the box and the number of
  *                      midpoints; n = 0 for a miss; or NULL
@@ -233,7 +239,7 @@ GDRR_API int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_be
  * caller's device scratch `signal_stage_dev` (>= min(proj_count, stage_proj) *
  * nv*nu floats, stage_proj >= 1 projections per batch) and copies each batch to
  * `signal_host` [proj_count][nv][nu]; returns after the last copy completed.
- * For overlap signal_host should be pinned. */
+ * For overlap signal_host should be pinned.  At most four materials (UNSUPPORTED otherwise). */
 GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
                       int proj_count, float* signal_host, float* signal_stage_dev,
                       int stage_proj, void* cuda_stream);

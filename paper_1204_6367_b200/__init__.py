@@ -33,7 +33,7 @@ GDRR_SAMPLER_STAGED = 2
 GDRR_METHOD_TRILINEAR = 0
 GDRR_METHOD_SIDDON = 1
 GDRR_METHOD_TEXTURE = 2
-GDRR_MAX_MATERIALS = 4
+GDRR_MAX_MATERIALS = 16
 GDRR_MAX_ENERGIES = 512
 
 EXPORTS = (
@@ -432,7 +432,7 @@ class Projector:
             if signal is None:
                 signal = torch.empty((n, w.nv, w.nu), dtype=torch.float32, device=self.device)
             li = (torch.empty((n, w.n_materials, w.nv, w.nu), dtype=torch.float32, device=self.device)
-                  if want_li else None)
+                  if want_li or w.n_materials > 4 else None)      # (more than four materials: required by the library)
             tab = (torch.empty((n, w.nv, w.nu, 2), dtype=torch.int32, device=self.device)
                    if want_table else None)
             gdrr_project(self.ctx, self.vol, proj_begin, n, signal, li, tab)

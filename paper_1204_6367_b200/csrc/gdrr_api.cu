@@ -33,7 +33,8 @@ struct gdrr_context {
     // spectrum
     bool has_spec = false;
     int n_energy = 0, n_mat = 0;
-    float4* mu_dev = nullptr;
+    float4* mu_dev = nullptr;       // [n_energy] log2(e) mu_hat of the first (up to) four materials
+    float* mu_all_dev = nullptr;    // [n_energy][n_mat] the same for all materials (more than four: energy_sum.cu)
     float2* src_dev = nullptr;
     float* bt_dev = nullptr;
     float* flu_dev = nullptr;
@@ -62,7 +63,11 @@ struct gdrr_volume {
     void* vox;
     int nx, ny, nz, px, py, pz;
     double d[3], c[3];
-    int n_mat, vw, layout;
+    // A volume of more than four materials is a chain of device volumes, one per group of four materials, each complete
+    // (its own layout, tensor map, compact copy); `groups` of the first one holds the others.  n_mat: the caller's
+    // count (on every member); this member holds materials [mat_lo, mat_lo + n_group).
+    int n_mat, n_group, mat_lo, vw, layout;
+    std::vector<gdrr_volume*> groups;
     int sy, sz;                 // PACKED_QUAD: element strides
     void* compact = nullptr;    // PACKED_QUAD: one-word-per-voxel copy, rows in groups of four (Siddon walk)
     // ... made from the quads at the first Siddon use: `compact_mu` serialises the callers, `compact_done` orders every
@@ -201,6 +206,8 @@ int volume_check(gdrr_context* ctx, const gdrr_volume* cvol, bool wait) {
     }
     if (vol->bad)
         return fail(ctx, GDRR_ERR_INVALID_ARG, "a material index of this volume is >= n_materials (%d)", vol->n_mat);
+    for (gdrr_volume* g : vol->groups)
+        if (int rc = volume_check(ctx, g, wait)) return rc;
     return GDRR_OK;
 }
 
@@ -246,18 +253,10 @@ int fill_geom(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int pro
     return GDRR_OK;
 }
 
-int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
-                 ProjectParams& P) {
-    int rc = fill_geom(ctx, vol, proj_begin, proj_count, P.g);
-    if (rc) return rc;
-    if (!ctx->has_spec) return fail(ctx, GDRR_ERR_NOT_READY, "gdrr_set_spectrum has not been called");
-    if (ctx->n_mat != vol->n_mat)
-        return fail(ctx, GDRR_ERR_NOT_READY, "spectrum has %d materials, volume has %d", ctx->n_mat, vol->n_mat);
-    if (ctx->method == GDRR_METHOD_TEXTURE && !vol->tex)
-        return fail(ctx, GDRR_ERR_NOT_READY, "GDRR_METHOD_TEXTURE needs gdrr_volume_attach_texture on this volume");
+// The device-volume part of the kernel parameters (one member of a chain of material groups).
+void fill_volume(const gdrr_volume* vol, ProjectParams& P) {
     P.v.vox = vol->vox;
     P.v.nvox[0] = vol->nx; P.v.nvox[1] = vol->ny; P.v.nvox[2] = vol->nz;
-    P.seg_table = nullptr;
     P.v.compact = vol->compact;
     P.v.cstride_y = 4 * vol->nx;
     P.v.cstride_z = 4 * vol->nx * ((vol->ny + 3) / 4);
@@ -272,13 +271,31 @@ int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
         P.v.stride_z = vol->px * vol->py;
     }
     P.v.vox1 = (const char*)vol->vox + 16 * (size_t)vol->sz;
+    P.n_mat = vol->n_group;
+    P.li_mat0 = vol->mat_lo;
+}
+
+int fill_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int proj_count,
+                 ProjectParams& P) {
+    int rc = fill_geom(ctx, vol, proj_begin, proj_count, P.g);
+    if (rc) return rc;
+    if (!ctx->has_spec) return fail(ctx, GDRR_ERR_NOT_READY, "gdrr_set_spectrum has not been called");
+    if (ctx->n_mat != vol->n_mat)
+        return fail(ctx, GDRR_ERR_NOT_READY, "spectrum has %d materials, volume has %d", ctx->n_mat, vol->n_mat);
+    if (ctx->method == GDRR_METHOD_TEXTURE && !vol->groups.empty())
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "GDRR_METHOD_TEXTURE holds at most four materials (four texture channels)");
+    if (ctx->method == GDRR_METHOD_TEXTURE && !vol->tex)
+        return fail(ctx, GDRR_ERR_NOT_READY, "GDRR_METHOD_TEXTURE needs gdrr_volume_attach_texture on this volume");
+    fill_volume(vol, P);
+    P.seg_table = nullptr;
     P.mu_tab = ctx->mu_dev;
     P.src_tab = ctx->src_dev;
     P.bt_thick = ctx->bt_dev;
     P.fluence = ctx->flu_dev;
     P.gain = ctx->gain_dev;
     P.n_energy = ctx->n_energy;
-    P.n_mat = ctx->n_mat;
+    P.li_only = 0; P.li_mat_total = vol->n_mat;
+    P.mu_all = ctx->mu_all_dev;
     // in-chunk positions are 9.23 fixed point: keep |advance| per chunk below 128 voxels
     double dgmax = 0.0;
     for (int a = 0; a < 3; ++a) dgmax = std::fmax(dgmax, P.g.step / vol->d[a]);
@@ -333,7 +350,7 @@ cudaError_t ensure_compact(const gdrr_volume* cvol, cudaStream_t s) {
         IngestParams ip = {};
         ip.vox = vol->vox; ip.compact = vol->compact;
         ip.nx = vol->nx; ip.ny = vol->ny; ip.nz = vol->nz;
-        ip.sy = vol->sy; ip.sz = vol->sz; ip.n_mat = vol->n_mat;
+        ip.sy = vol->sy; ip.sz = vol->sz; ip.n_mat = vol->n_mat; ip.tagged = vol->n_group > 1;
         ip.cbx = (vol->nx + 3) / 4; ip.cby = (vol->ny + 3) / 4;
         e = launch_compact_copy(ip, s);
         if (e == cudaSuccess) e = cudaEventRecord(vol->compact_done, s);
@@ -346,9 +363,11 @@ cudaError_t ensure_compact(const gdrr_volume* cvol, cudaStream_t s) {
 
 // Does staging pay?  Extent, in voxels per axis, of the beam of a 16 x 16-pixel CTA over 16 steps at the
 // depth of the box centre, averaged over the requested projections, against the 14 x 14 x 11-quad box (a chunk
-// whose beam does not fit is gathered anyway, after paying for its bounding box).  Thresholds measured on C3
-// (staged against gather): circle and helix (mean extents 10.5, 10.5, 6.6) +19%; orbit tilted 10 degrees
-// (10.5, 11.8, 8.0) +22%; tilted 20 degrees (10.5, 12.7, 9.0) -2%; tilted 35 degrees (10.5, 13.4, 10.1) -20%.
+// whose beam does not fit is gathered anyway, after its box has been refused).  Thresholds measured on C3 with the
+// round-2 kernels (staged against gather, samples/s): circle and helix (mean extents 10.5, 10.5, 6.6) 7.39e11 against
+// 5.03e11; orbit tilted 10 degrees (10.5, 11.8, 8.0) 6.75e11 against 4.95e11; tilted 20 degrees (10.5, 12.7, 9.0)
+// 5.58e11 against 4.91e11; tilted 35 degrees (10.5, 13.4, 10.1) 4.50e11 against 4.90e11: the line is drawn halfway
+// between the last two.  tests/test_gpu_sampler_choice.py pins what AUTO picks on each of these.
 bool beam_fits(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& g) {
     double ext[3] = {0.0, 0.0, 0.0};
     for (int p = g.proj_begin; p < g.proj_begin + g.proj_count; ++p) {
@@ -369,7 +388,7 @@ bool beam_fits(const gdrr_context* c, const gdrr_volume* vol, const GeomParams& 
                        16.0 * g.step * std::fabs(P[a] - S[a]) / std::sqrt(sp)) / vol->d[a];
     }
     for (int a = 0; a < 3; ++a) ext[a] /= (double)g.proj_count;
-    return ext[0] <= 12.5 && ext[1] <= 12.5 && ext[2] <= 8.9;
+    return ext[0] <= 13.05 && ext[1] <= 13.05 && ext[2] <= 9.55;
 }
 
 // The staged sampler bounds a chunk of a CTA's beam by its four CORNER rays (project_staged.cu).  How far can a ray of
@@ -425,7 +444,25 @@ cudaError_t order_after_ingest(const gdrr_volume* vol, cudaStream_t s) {
     return cudaStreamWaitEvent(s, vol->ingest_done, 0);
 }
 
+cudaError_t launch_one(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s);
+
+// One launch for up to four materials.  More: one LI-only launch per group of four (each on its own device volume, the
+// ray table written once), then the energy sum over all line integrals (energy_sum.cu); P.li is required then.
 cudaError_t launch_project(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
+    if (vol->groups.empty()) return launch_one(P, vol, s);
+    ProjectParams Pg = P;
+    Pg.li_only = 1;
+    for (size_t g = 0; g <= vol->groups.size(); ++g) {
+        const gdrr_volume* member = g == 0 ? vol : vol->groups[g - 1];
+        fill_volume(member, Pg);
+        if (g > 0) Pg.ray_table = nullptr;
+        if (cudaError_t e = launch_one(Pg, member, s)) return e;
+        vol->ctx->launches += 1;
+    }
+    return launch_energy_sum(P, s);          // (the caller counts this last launch)
+}
+
+cudaError_t launch_one(const ProjectParams& P, const gdrr_volume* vol, cudaStream_t s) {
     gdrr_context* c = vol->ctx;
     if (cudaError_t e = order_after_ingest(vol, s)) return e;
     if (c->method == GDRR_METHOD_SIDDON) {
@@ -488,7 +525,7 @@ int gdrr_destroy_context(gdrr_context* ctx) {
     if (!ctx) return GDRR_OK;
     DeviceGuard guard(ctx->device);
     free_dev(ctx->poses_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
-    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->gain_dev);
+    free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->gain_dev); free_dev(ctx->mu_all_dev);
     if (ctx->flag_host) { cudaFreeHost(ctx->flag_host); ctx->flag_host = nullptr; ctx->flag_dev = nullptr; }
     for (int k = 0; k < 2; ++k) {
         if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
@@ -508,20 +545,35 @@ const char* gdrr_last_error(const gdrr_context* ctx) {
 
 unsigned long long gdrr_kernel_launches(const gdrr_context* ctx) { return ctx ? ctx->launches : 0ull; }
 
+// Workspace of ONE device volume holding n_group (<= 4) materials, rounded up to 256 bytes.
+static size_t group_workspace_bytes(int nx, int ny, int nz, int n_group, int layout) {
+    int px, py, pz;
+    stored_dims(nx, ny, nz, layout, px, py, pz);
+    size_t bytes = (size_t)px * py * pz * element_bytes(n_group, layout);
+    if (layout == GDRR_LAYOUT_PACKED_QUAD)
+        bytes = ((16 * packed_elements(nx, ny, nz) + 255) & ~(size_t)255) + compact_bytes(nx, ny, nz);
+    return (bytes + 255) & ~(size_t)255;
+}
+
 int gdrr_volume_workspace_bytes(int nx, int ny, int nz, int n_materials, int layout, size_t* bytes) {
     if (!bytes) return fail(nullptr, GDRR_ERR_INVALID_ARG, "bytes is NULL");
     int rc = check_dims(nullptr, nx, ny, nz, n_materials, layout);
     if (rc) return rc;
-    int px, py, pz;
-    stored_dims(nx, ny, nz, layout, px, py, pz);
-    *bytes = (size_t)px * py * pz * element_bytes(n_materials, layout);
-    if (layout == GDRR_LAYOUT_PACKED_QUAD) *bytes = ((16 * packed_elements(nx, ny, nz) + 255) & ~(size_t)255) + compact_bytes(nx, ny, nz);
+    *bytes = 0;
+    for (int lo = 0; lo < n_materials; lo += 4)          // one device volume per group of four materials
+        *bytes += group_workspace_bytes(nx, ny, nz, std::min(4, n_materials - lo), layout);
     return GDRR_OK;
 }
 
 // gdrr_create_volume and gdrr_create_volume_host.  rho_host / mat_host != NULL: the inputs are first copied into
 // rho_dev / mat_dev (the caller's staging buffers) in z-slab chunks on the context's copy stream, and the slabs of the
 // device layout that a chunk completes are written while the next chunk is still on the bus.
+static int create_group(gdrr_context* ctx, const float* rho_host, const uint8_t* mat_host,
+                        float* rho_dev, uint8_t* mat_dev, int nx, int ny, int nz,
+                        double dx_mm, double dy_mm, double dz_mm, const double centre_mm[3], int n_materials,
+                        int mat_lo, int n_group, int layout, void* workspace_dev, void* cuda_stream, gdrr_volume** out);
+
+// All groups of four materials, chained behind the first (the only one that copies from the host).
 static int create_volume_impl(gdrr_context* ctx, const float* rho_host, const uint8_t* mat_host,
                               float* rho_dev, uint8_t* mat_dev, int nx, int ny, int nz,
                               double dx_mm, double dy_mm, double dz_mm, const double centre_mm[3], int n_materials,
@@ -537,7 +589,28 @@ static int create_volume_impl(gdrr_context* ctx, const float* rho_host, const ui
         return fail(ctx, GDRR_ERR_WORKSPACE, "workspace of %zu bytes given, %zu needed", workspace_bytes, need);
     if ((uintptr_t)workspace_dev % 256)
         return fail(ctx, GDRR_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+    gdrr_volume* first = nullptr;
+    char* ws = (char*)workspace_dev;
+    for (int lo = 0; lo < n_materials; lo += 4) {
+        const int n_group = std::min(4, n_materials - lo);
+        gdrr_volume* v = nullptr;
+        int rc = create_group(ctx, lo == 0 ? rho_host : nullptr, lo == 0 ? mat_host : nullptr, rho_dev, mat_dev, nx, ny, nz,
+                              dx_mm, dy_mm, dz_mm, centre_mm, n_materials, lo, n_group, layout, ws, cuda_stream, &v);
+        if (rc) {
+            if (first) gdrr_destroy_volume(first);
+            return rc;
+        }
+        if (first) first->groups.push_back(v); else first = v;
+        ws += group_workspace_bytes(nx, ny, nz, n_group, layout);
+    }
+    *out = first;
+    return GDRR_OK;
+}
 
+static int create_group(gdrr_context* ctx, const float* rho_host, const uint8_t* mat_host,
+                        float* rho_dev, uint8_t* mat_dev, int nx, int ny, int nz,
+                        double dx_mm, double dy_mm, double dz_mm, const double centre_mm[3], int n_materials,
+                        int mat_lo, int n_group, int layout, void* workspace_dev, void* cuda_stream, gdrr_volume** out) {
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -554,13 +627,14 @@ static int create_volume_impl(gdrr_context* ctx, const float* rho_host, const ui
     ip.nx = nx; ip.ny = ny; ip.nz = nz;
     stored_dims(nx, ny, nz, layout, ip.px, ip.py, ip.pz);
     ip.n_mat = n_materials; ip.bad_flag = ctx->flag_dev + slot;
+    ip.mat_lo = mat_lo; ip.n_group = n_group; ip.tagged = n_group > 1;
     ip.sy = ip.sz = 0;
     ip.compact = nullptr; ip.cbx = (nx + 3) / 4; ip.cby = (ny + 3) / 4;
     if (layout == GDRR_LAYOUT_PACKED_QUAD) {
         packed_strides(ip.px, ip.py, ip.sy, ip.sz);
         ip.compact = (char*)workspace_dev + ((16 * (size_t)ip.sz * ip.pz + 255) & ~(size_t)255);
     }
-    const int vw = vector_width(n_materials);
+    const int vw = vector_width(n_group);
     const size_t slab = (size_t)nx * ny;
     // chunks of whole z slabs, at least ~4 MB of rho each; BRICK stores 2 x 2 x 2 bricks: one chunk
     int chunks = 1;
@@ -609,7 +683,7 @@ static int create_volume_impl(gdrr_context* ctx, const float* rho_host, const ui
     v->nx = nx; v->ny = ny; v->nz = nz; v->px = ip.px; v->py = ip.py; v->pz = ip.pz;
     v->d[0] = dx_mm; v->d[1] = dy_mm; v->d[2] = dz_mm;
     for (int a = 0; a < 3; ++a) v->c[a] = centre_mm ? centre_mm[a] : 0.0;
-    v->n_mat = n_materials; v->vw = vw; v->layout = layout;
+    v->n_mat = n_materials; v->n_group = n_group; v->mat_lo = mat_lo; v->vw = vw; v->layout = layout;
     v->sy = ip.sy; v->sz = ip.sz; v->compact = ip.compact;
     v->has_tmap = layout == GDRR_LAYOUT_PACKED_QUAD && make_tensor_map(v);
     *out = v;
@@ -656,6 +730,8 @@ int gdrr_volume_status(gdrr_context* ctx, const gdrr_volume* vol) {
 }
 
 int gdrr_destroy_volume(gdrr_volume* vol) {
+    if (vol)
+        for (gdrr_volume* g : vol->groups) gdrr_destroy_volume(g);
     if (vol && (vol->tex || vol->tex_array || vol->compact_done || vol->ingest_done)) {
         DeviceGuard guard(vol->ctx->device);
         if (vol->ingest_done) cudaEventDestroy(vol->ingest_done);
@@ -777,12 +853,21 @@ int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,
     std::vector<float2> src((size_t)n_energy);
     for (int e = 0; e < n_energy; ++e) {
         float m4[4] = {0.f, 0.f, 0.f, 0.f};
-        for (int m = 0; m < n_materials; ++m) m4[m] = (float)(log2e * mu_hat[(size_t)m * n_energy + e]);
+        for (int m = 0; m < n_materials && m < 4; ++m) m4[m] = (float)(log2e * mu_hat[(size_t)m * n_energy + e]);
         mu[e] = make_float4(m4[0], m4[1], m4[2], m4[3]);
         src[e] = make_float2((float)(phi_weight[e] * response[e]), bowtie_mu ? (float)(log2e * bowtie_mu[e]) : 0.f);
     }
     float4* mu_dev = nullptr; float2* src_dev = nullptr; float* bt_dev = nullptr; float* flu_dev = nullptr;
+    float* mu_all_dev = nullptr;
     cudaError_t e = cudaMalloc(&mu_dev, sizeof(float4) * n_energy);
+    if (e == cudaSuccess && n_materials > 4) {       // the energy sum over more than four materials reads [E][M]
+        std::vector<float> all((size_t)n_energy * n_materials);
+        for (int en = 0; en < n_energy; ++en)
+            for (int m = 0; m < n_materials; ++m)
+                all[(size_t)en * n_materials + m] = (float)(log2e * mu_hat[(size_t)m * n_energy + en]);
+        e = cudaMalloc(&mu_all_dev, sizeof(float) * all.size());
+        if (e == cudaSuccess) e = cudaMemcpy(mu_all_dev, all.data(), sizeof(float) * all.size(), cudaMemcpyHostToDevice);
+    }
     if (e == cudaSuccess) e = cudaMalloc(&src_dev, sizeof(float2) * n_energy);
     if (e == cudaSuccess) e = cudaMemcpy(mu_dev, mu.data(), sizeof(float4) * n_energy, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(src_dev, src.data(), sizeof(float2) * n_energy, cudaMemcpyHostToDevice);
@@ -798,12 +883,13 @@ int gdrr_set_spectrum(gdrr_context* ctx, int n_energy, int n_materials,
         if (e == cudaSuccess) e = cudaMemcpy(flu_dev, fluence_map, sizeof(float) * n, cudaMemcpyHostToDevice);
     }
     if (e != cudaSuccess) {
-        free_dev(mu_dev); free_dev(src_dev); free_dev(bt_dev); free_dev(flu_dev);
+        free_dev(mu_dev); free_dev(src_dev); free_dev(bt_dev); free_dev(flu_dev); free_dev(mu_all_dev);
         return cuda_fail(ctx, e, "uploading the spectrum tables");
     }
     free_dev(ctx->mu_dev); free_dev(ctx->src_dev); free_dev(ctx->bt_dev); free_dev(ctx->flu_dev);
     if (n_energy != ctx->n_energy) free_dev(ctx->gain_dev);        // shaped by the old energy grid
-    ctx->mu_dev = mu_dev; ctx->src_dev = src_dev; ctx->bt_dev = bt_dev; ctx->flu_dev = flu_dev;
+    free_dev(ctx->mu_all_dev);
+    ctx->mu_dev = mu_dev; ctx->src_dev = src_dev; ctx->bt_dev = bt_dev; ctx->flu_dev = flu_dev; ctx->mu_all_dev = mu_all_dev;
     ctx->n_energy = n_energy; ctx->n_mat = n_materials;
     ctx->has_spec = true;
     return GDRR_OK;
@@ -837,6 +923,9 @@ int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin, int 
     int rc = fill_project(ctx, vol, proj_begin, proj_count, P);
     if (rc) return rc;
     P.signal = signal_dev; P.li = line_integrals_dev; P.ray_table = ray_table_dev;
+    if (!vol->groups.empty() && !line_integrals_dev)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "with more than four materials gdrr_project needs line_integrals_dev: the line "
+                    "integrals of each group of four wait there for the energy sum");
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaError_t e = launch_project(P, vol, (cudaStream_t)cuda_stream);
@@ -853,6 +942,9 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
     ProjectParams P;
     int rc = fill_project(ctx, vol, proj_begin, proj_count, P);
     if (rc) return rc;
+    if (!vol->groups.empty())
+        return fail(ctx, GDRR_ERR_UNSUPPORTED, "gdrr_project_host holds at most four materials (no scratch for the line "
+                    "integrals of the groups): use gdrr_project with line_integrals_dev");
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaStream_t s = (cudaStream_t)cuda_stream;

@@ -54,7 +54,12 @@ struct ProjectParams {
     const float* bt_thick;          // [nu] or nullptr
     const float* fluence;           // [nv][nu] or nullptr
     const float* gain;              // [n_energy][nv][nu] pixel-dependent response gain g(E, u) or nullptr (reading Q32)
-    int n_energy, n_mat;
+    int n_energy, n_mat;            // n_mat: materials of THIS device volume (<= 4; a group of the caller's materials)
+    // more than four materials: the volume is kept as groups of four (gdrr_api.cu); a launch then only writes its
+    // group's line integrals (li_only) at material offset li_mat0 of the caller's [proj][li_mat_total][nv][nu] array,
+    // and gdrr_energy_sum_kernel forms the signal from all of them with mu_all
+    int li_only, li_mat0, li_mat_total;
+    const float* mu_all;            // [n_energy][li_mat_total] log2(e) * mu_hat, or nullptr (<= 4 materials)
     int chunk;                      // <= kMaxChunk
     unsigned frac_mask, one_bits;   // 0x007FFFFF, 0x3F800000: kept in registers by the samplers
     // staged sampler: bound, in voxels per axis, on how far a ray of a 16 x 16-pixel tile can lie outside the hull of
@@ -78,7 +83,10 @@ struct IngestParams {
     int sy, sz;                     // PACKED_QUAD: element strides (VolumeParams)
     void* compact;                  // PACKED_QUAD: the one-word-per-voxel copy, rows in groups of four
     int cbx, cby;                   //   ceil(nx / 4), ceil(ny / 4) (cby: groups of four rows per slab)
-    int n_mat;
+    int n_mat;                      // the caller's material count: an index >= n_mat raises bad_flag
+    int mat_lo, n_group;            // this device volume holds materials [mat_lo, mat_lo + n_group) as tags 0..n_group-1;
+                                    // voxels of other materials are stored as rho = 0 (tag 0): they add nothing to any sum
+    int tagged;                     // PACKED_QUAD: words carry tags (n_group > 1)
     int* bad_flag;                  // set to 1 if a material index >= n_mat is seen
 };
 
@@ -99,6 +107,8 @@ cudaError_t launch_debug_ray_cells(const ProjectParams& p, int i, int j, int sta
 cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
                              unsigned long long* n_samples, cudaStream_t s);
 
+// more than four materials: signal from the line integrals of all groups (energy_sum.cu)
+cudaError_t launch_energy_sum(const ProjectParams& p, cudaStream_t s);
 cudaError_t launch_denoise(const float* s_hat, float* s_dev, float* scratch, int nu, int nv, int n_images,
                            double beta, double omega, int n_iter, double floor_value, cudaStream_t st, int* launches);
 

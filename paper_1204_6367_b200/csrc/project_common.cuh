@@ -68,11 +68,12 @@ __device__ __forceinline__ void finish_pixel(const ProjectParams& P, const float
     for (int m = 0; m < VW; ++m) li[m] = (float)((double)acc[m] * scale);
     if (P.li) {
         const size_t plane = (size_t)P.g.nv * P.g.nu;
-        float* o = P.li + (size_t)pl * P.n_mat * plane + (size_t)j * P.g.nu + i;
+        float* o = P.li + ((size_t)pl * P.li_mat_total + P.li_mat0) * plane + (size_t)j * P.g.nu + i;
 #pragma unroll
         for (int m = 0; m < VW; ++m)
             if (m < P.n_mat) o[m * plane] = li[m];
     }
+    if (P.li_only) return;          // one group of more than four materials: gdrr_energy_sum_kernel forms the signal
     const float tb = P.bt_thick ? P.bt_thick[i] : 0.f;
     // pixel-dependent detector response r(E, u) = r(E) g(E, u) (reading Q32): g streams in from global
     // memory, energy-major, so that the pixels of a warp read neighbouring words

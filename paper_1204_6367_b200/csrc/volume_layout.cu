@@ -57,10 +57,12 @@ gdrr_ingest_kernel(const IngestParams P) {
     const int iy = min(max(sy_ - 1, 0), P.ny - 1);
     const int iz = min(max(sz_ - 1, 0), P.nz - 1);
     const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
-    const float rho = P.rho[src];
     const int m = P.mat[src];
     if (m >= P.n_mat) *P.bad_flag = 1;
-    reinterpret_cast<V*>(P.vox)[o] = one_hot<VW>(rho, m);
+    // a voxel whose material belongs to another group of four is an empty voxel of this device volume
+    const int local = m - P.mat_lo;
+    const bool here = (unsigned)local < (unsigned)P.n_group;
+    reinterpret_cast<V*>(P.vox)[o] = one_hot<VW>(here ? P.rho[src] : 0.f, here ? local : 0);
 }
 
 // PACKED_QUAD (project_packed.cu): element (ex, ey, ez) = the four words of stored
@@ -93,20 +95,23 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
                 const int ix = min(max(ex + (k >> 1) - 1, 0), P.nx - 1);
                 const int iy = min(max(ey + (k & 1) - 1, 0), P.ny - 1);
                 const size_t src = ((size_t)iz * P.ny + iy) * P.nx + ix;
-                const unsigned m = P.mat[src];
+                const unsigned mg = P.mat[src];
+                if ((int)mg >= P.n_mat) *P.bad_flag = 1;
+                // a voxel whose material belongs to another group of four is an empty voxel (tag 0) of this device volume
+                const bool here = mg - (unsigned)P.mat_lo < (unsigned)P.n_group;
+                const unsigned m = here ? mg - (unsigned)P.mat_lo : 0u;
                 if (dz == 0 && k == 0) m0 = m;
                 mixed |= m ^ m0;
                 seen |= 1u << (m & 3u);
                 if (dz == 0) {
-                    unsigned bits = __float_as_uint(P.rho[src]);
-                    if ((int)m >= P.n_mat) *P.bad_flag = 1;
-                    if (P.n_mat > 1) bits = ((bits + 4u) & ~7u) | (m & 3u);
+                    unsigned bits = here ? __float_as_uint(P.rho[src]) : 0u;
+                    if (P.tagged) bits = ((bits + 4u) & ~7u) | (m & 3u);
                     w[k] = bits;
                 }
             }
         }
-        if (P.n_mat > 1 && mixed == 0u) w[0] |= 4u;
-        if (P.n_mat > 1 && __popc(seen) == 2) {
+        if (P.tagged && mixed == 0u) w[0] |= 4u;
+        if (P.tagged && __popc(seen) == 2) {
             const unsigned q = (unsigned)(__ffs((int)(seen & ~(1u << (m0 & 3u)))) - 1);     // the other material
             w[1] |= 4u;
             w[2] |= (q & 1u) << 2;
@@ -135,7 +140,7 @@ gdrr_ingest_compact_kernel(const IngestParams P) {
     if (iy < P.ny) {
         // voxel (ix, iy, iz) is the first word of quad (ix + 1, iy + 1, iz + 1); drop its purity flag
         bits = reinterpret_cast<const unsigned*>(P.vox)[4 * ((size_t)(iz + 1) * P.sz + (size_t)(iy + 1) * P.sy + (ix + 1))];
-        if (P.n_mat > 1) bits &= ~4u;
+        if (P.tagged) bits &= ~4u;
     }
     reinterpret_cast<unsigned*>(P.compact)[((size_t)iz * P.cby + blockIdx.y) * (4 * (size_t)P.nx) + t] = bits;
 }

@@ -44,8 +44,10 @@ def test_host_only_calls_return_status_codes():
     with pytest.raises(g.GdrrError) as e:
         g.gdrr_volume_workspace_bytes(0, 4, 4, 1, g.GDRR_LAYOUT_LINEAR)
     assert e.value.code == g.GDRR_ERR_INVALID_ARG
+    # more than four materials: one device volume per group of four (here 4 + 1 materials: float4 + float per voxel)
+    assert g.gdrr_volume_workspace_bytes(30, 30, 30, 5, g.GDRR_LAYOUT_LINEAR) == 32 * 32 * 32 * (16 + 4)
     with pytest.raises(g.GdrrError) as e:
-        g.gdrr_volume_workspace_bytes(8, 8, 8, 5, g.GDRR_LAYOUT_LINEAR)
+        g.gdrr_volume_workspace_bytes(8, 8, 8, g.GDRR_MAX_MATERIALS + 1, g.GDRR_LAYOUT_LINEAR)
     assert e.value.code == g.GDRR_ERR_UNSUPPORTED
     with pytest.raises(g.GdrrError) as e:
         g.gdrr_volume_workspace_bytes(8, 8, 8, 1, 7)

@@ -40,7 +40,7 @@ def test_auto_choice_on_other_source_paths(gdrr, workloads_cache):
     nz_mm = w.dims[2] * w.spacing[2]
     helix = w.with_poses(trajectories.helical_poses(w.sad, w.sdd, phis, pitch_mm=0.5 * nz_mm, z0_mm=-0.25 * nz_mm))
     assert _picked(gdrr, helix) == gdrr.GDRR_SAMPLER_STAGED
-    for tilt, want in ((10.0, "STAGED"), (20.0, "GATHER"), (35.0, "GATHER")):
+    for tilt, want in ((10.0, "STAGED"), (20.0, "STAGED"), (35.0, "GATHER")):
         tilted = w.with_poses(trajectories.c_arm_poses(w.sad, w.sdd, phis, np.deg2rad(tilt)))
         assert _picked(gdrr, tilted) == getattr(gdrr, "GDRR_SAMPLER_" + want), tilt
     # an explicit choice is honoured; exact layouts report 0
