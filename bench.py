@@ -260,6 +260,10 @@ def run_b200(args):
         w = w0.with_phis(gd.scan_angles(n_total)[mine])
     else:                                                   # profiling aid: every projection at one angle
         w = w0.with_phis(np.full(per_gpu, np.deg2rad(args.angle_deg)))
+    if args.u_off_mm:                                       # half-fan scan (detector shifted along u)
+        import copy
+        w = copy.copy(w)
+        w.u_off = float(args.u_off_mm)
     if args.trajectory != "circle":                         # other source paths, same kernels
         from workloads import trajectories
         nz_mm = w.dims[2] * w.spacing[2]
@@ -382,7 +386,8 @@ def run_b200(args):
     l1_peak = SM_COUNT * L1_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9       # GB/s
     l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
     # what only ncu can see comes from the committed capture of these very sources, or is None (never a stale constant)
-    ncu = ncu_constants(kname, args.workload if args.phantom == "smooth" and args.trajectory == "circle" else "-")
+    ncu = ncu_constants(kname, args.workload if args.phantom == "smooth" and args.trajectory == "circle"
+                        and not args.u_off_mm else "-")
     dram_step = ncu["dram_bytes_per_projection"] * per_gpu if ncu["dram_bytes_per_projection"] else None
     # the least a projection must move: every voxel of its cone once as a 4-byte word, and its image
     hbm_min = None
@@ -427,7 +432,7 @@ def run_b200(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
             "config": dict(workload_config(w, args.workload, world, n_total, launch_proj),
-                           phantom=args.phantom, pure_cell_fraction=pure_cell_fraction(w.mat),
+                           phantom=args.phantom, pure_cell_fraction=pure_cell_fraction(w.mat), u_off_mm=w.u_off,
                            inputs_sha256=w.sha256(),
                            **({} if args.trajectory == "circle" else {"trajectory": args.trajectory})),
             "projections_per_s": proj_per_s, "samples_per_step": total_samples,
@@ -533,6 +538,8 @@ def main():
                     help="source path: the paper's circle (the headline), a one-turn helix over half the volume's "
                          "height, or the circle tilted about x by --tilt-deg (gdrr_set_geometry_poses)")
     ap.add_argument("--tilt-deg", type=float, default=20.0)
+    ap.add_argument("--u-off-mm", type=float, default=0.0,
+                    help="detector offset along u (half-fan scan: e.g. 148 on C3, where the far rays cross a corner of the volume)")
     ap.add_argument("--phantom", default="smooth", choices=["smooth", "noisy1", "noisy3", "random"],
                     help="C2..C4: the BASELINE recipe (smooth), the same with 1 % / 3 % voxel noise before the material "
                          "thresholds, or materials drawn per voxel (workloads/configs.py); the pure-cell fraction is printed")

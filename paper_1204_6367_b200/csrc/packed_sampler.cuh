@@ -113,12 +113,8 @@ __device__ __forceinline__ void switch_material(RayAcc<VW>& A, unsigned m4) {
 template <int VW>
 __device__ __forceinline__ void blend_general(const uint4& a, const uint4& c, float fx, float fy, float fz, float v,
                                               RayAcc<VW>& A) {
-    if (a.x & 4u) {
-        // pure cell of another material: the running sum moves there
-        switch_material<VW>(A, a.x & 7u);
-        A.cur = v;
-        return;
-    }
+    // (the two-material test comes first: in a noisy volume it is what most lanes that get here need, and the arms
+    // of this chain are short enough for ptxas to predicate, so a later arm costs every lane of an earlier one nothing)
     const unsigned p = a.x & 3u;
     if (a.y & 4u) {
         // two materials p and q: one more blend of the corners of material p alone (the others as 0), the rest is q's
@@ -135,6 +131,10 @@ __device__ __forceinline__ void blend_general(const uint4& a, const uint4& c, fl
         const unsigned q = ((a.z >> 2) & 1u) | ((a.w >> 1) & 2u);
         route<VW>(A, p, vp);
         route<VW>(A, q, v - vp);
+    } else if (a.x & 4u) {
+        // pure cell of another material: the running sum moves there
+        switch_material<VW>(A, a.x & 7u);
+        A.cur = v;
     } else {
         // three or four materials: route every weighted corner
         const float gx = 1.f - fx, gy = 1.f - fy, gz = 1.f - fz;
