@@ -104,6 +104,19 @@ def test_both_packed_samplers_against_the_oracle(gdrr, workloads_cache, sampler)
             compare_full(pr, ws, oracle.project(ws), f"step {step} sampler {sampler}")
 
 
+@pytest.mark.parametrize("phantom", ["noisy3", "random"])
+@pytest.mark.parametrize("sampler", [1, 2])
+def test_c2_phantom_variants_full_image(gdrr, phantom, sampler):
+    """The mixed-cell paths at clinical size: C2 with 3 % voxel noise before the material thresholds (13 % of its cells
+    mix two materials: the masked second blend) and with a material drawn per voxel (every cell mixes three or four:
+    the routed corners), every pixel of a projection at 37 degrees against the oracle, both samplers."""
+    w = make_workload("C2", phantom=phantom).with_phis([math.radians(37.0)])
+    ref = oracle.project(w)
+    with gdrr.Projector(w, sampler=sampler) as pr:
+        stats = compare_full(pr, w, ref, f"C2 {phantom} sampler {sampler}")
+    print(phantom, sampler, stats)
+
+
 def test_staged_and_gather_samplers_agree(gdrr, workloads_cache):
     """Same samples, same blend; only the summation chunks (16 vs 32) and the re-basing of the position differ."""
     w = workloads_cache("C2").with_phis(np.radians([0.0, 37.0, 211.0]))

@@ -383,6 +383,25 @@ def test_p8_material_routing_and_linearity(workloads_cache):
     assert np.array_equal(d["line_integrals"][:, ::-1], a["line_integrals"])
 
 
+def test_p8_many_materials_are_the_line_integrals_of_the_masked_fields():
+    """Up to 16 materials (reading Q33): LI_m of a volume of 11 materials equals the line integral of the
+    one-material volume rho * [mat == m], for every m -- the linearity the CUDA path's groups of four rest on."""
+    rng = np.random.default_rng(21)
+    shape = (10, 12, 14)
+    rho = rng.uniform(0.1, 2.0, size=shape).astype(np.float32)
+    mat = rng.integers(0, 11, size=shape).astype(np.uint8)
+    kw = dict(spacing=(2.0, 2.5, 3.0), nu=20, nv=16, du=3.0, dv=3.0, phis=np.radians([20.0, 200.0]), step=0.7)
+    w = tiny_workload(rho, mat, n_materials=11, mu_hat=rng.uniform(0.01, 0.05, size=(11, 1)), **kw)
+    full = oracle.project(w)
+    tau = np.zeros_like(full["signal"])
+    for m in range(11):
+        one = tiny_workload(np.where(mat == m, rho, np.float32(0.0)), **kw)
+        li_m = oracle.project(one)["line_integrals"][:, 0]
+        np.testing.assert_allclose(full["line_integrals"][:, m], li_m, rtol=1e-12, atol=1e-12)
+        tau += w.mu_hat[m, 0] * li_m
+    np.testing.assert_allclose(full["signal"], np.exp(-tau), rtol=1e-12)
+
+
 @pytest.mark.parametrize("name,npix", [("C0", 60), ("C1", 40), ("C2", 12)])
 def test_p8_paper_literal_form_equals_factored_form(workloads_cache, name, npix):
     """O5' (one trace per energy channel on mu_E = rho*mu_hat[mat][E], as the
