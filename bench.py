@@ -96,12 +96,13 @@ class ClockSampler:
 
 
 def source_digest():
-    """sha256 over the CUDA sources: the stamp that ties profiles/ncu_constants.json to the kernels it was captured on."""
+    """sha256 over the DEVICE sources (every file of csrc/ but the host-side gdrr_api.cu): the stamp that ties
+    profiles/ncu_constants.json to the kernels it was captured on."""
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_1204_6367_b200", "csrc")
     for name in sorted(os.listdir(csrc)):
-        if name.endswith((".cu", ".cuh", ".h")):
+        if name.endswith((".cu", ".cuh", ".h")) and name != "gdrr_api.cu":
             with open(os.path.join(csrc, name), "rb") as f:
                 h.update(name.encode() + b"\0" + f.read())
     return h.hexdigest()

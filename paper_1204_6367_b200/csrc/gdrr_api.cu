@@ -5,6 +5,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -79,7 +80,7 @@ struct gdrr_volume {
     // the device-side material check is read when the ingest has finished, never waited for (volume_check)
     cudaEvent_t ingest_done = nullptr;
     volatile int* bad_flag = nullptr;    // this volume's slot of ctx->flag_host
-    bool checked = false, bad = false;
+    std::atomic<bool> checked{false}, bad{false};   // (two threads may both read the verdict: they write the same values)
     cudaArray_t tex_array = nullptr;     // optional texture variant (gdrr_volume_attach_texture)
     cudaTextureObject_t tex = 0;
     alignas(64) CUtensorMap tmap;
@@ -196,8 +197,8 @@ int volume_check(gdrr_context* ctx, const gdrr_volume* cvol, bool wait) {
         DeviceGuard guard(ctx->device);
         cudaError_t e = wait ? cudaEventSynchronize(vol->ingest_done) : cudaEventQuery(vol->ingest_done);
         if (e == cudaSuccess) {
-            vol->bad = *vol->bad_flag != 0;
-            vol->checked = true;
+            vol->bad.store(*vol->bad_flag != 0);
+            vol->checked.store(true);
         } else if (e != cudaErrorNotReady) {
             return cuda_fail(ctx, e, "waiting for the volume ingest");
         } else {
