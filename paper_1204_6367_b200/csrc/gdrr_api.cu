@@ -637,11 +637,12 @@ static int create_group(gdrr_context* ctx, const float* rho_host, const uint8_t*
     }
     const int vw = vector_width(n_group);
     const size_t slab = (size_t)nx * ny;
-    // chunks of whole z slabs, at least ~4 MB of rho each; BRICK stores 2 x 2 x 2 bricks: one chunk
+    // chunks of whole z slabs, at least ~8 MB of rho each (a chunk costs four API calls: below that the host's
+    // time per chunk shows); BRICK stores 2 x 2 x 2 bricks: one chunk
     int chunks = 1;
     if (rho_host && layout != GDRR_LAYOUT_BRICK)
         chunks = (int)std::max<size_t>(1, std::min<size_t>({(size_t)gdrr_context::kIngestChunks, (size_t)nz,
-                                                             slab * nz * sizeof(float) / (4u << 20)}));
+                                                             slab * nz * sizeof(float) / (8u << 20)}));
     if (rho_host) {
         if (!ctx->copy_stream) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
         for (int k = 0; k < gdrr_context::kIngestChunks && e == cudaSuccess; ++k)
