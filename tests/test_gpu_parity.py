@@ -264,6 +264,28 @@ def test_edge_cases(gdrr, case, layout):
     print(case, layout, stats)
 
 
+@pytest.mark.parametrize("n_energy", [1, 7, 512])
+def test_energy_grid_sizes_up_to_the_maximum(gdrr, n_energy):
+    """1, an odd number and GDRR_MAX_ENERGIES = 512 energy bins (the tables then take 12 KB of every CTA's shared memory:
+    the staged kernel runs two CTAs per SM instead of three), three materials, every layout and sampler."""
+    rng = np.random.default_rng(n_energy)
+    rho, mat = _random_volume(rng, (18, 22, 26), 3)
+    energies = np.linspace(20.0, 140.0, n_energy) if n_energy > 1 else np.array([60.0])
+    w = tiny_workload(rho, mat, n_materials=3, spacing=(1.0, 1.2, 1.4), nu=44, nv=38, du=0.9, dv=0.9,
+                      phis=np.radians([12.0, 200.0]), step=0.45, energies=energies,
+                      mu_hat=rng.uniform(0.01, 0.05, size=(3, n_energy)),
+                      phi_weight=rng.dirichlet(np.ones(n_energy)), response=energies / 60.0)
+    w.bowtie_mu = rng.uniform(0.02, 0.08, size=n_energy)
+    w.bowtie_thickness = rng.uniform(1.0, 10.0, size=w.nu)
+    ref = oracle.project(w)
+    for layout, sampler in ((2, 1), (2, 2), (0, 0), (1, 0)):
+        with gdrr.Projector(w, layout=layout, sampler=sampler) as pr:
+            compare_full(pr, w, ref, f"{n_energy} bins layout {layout} sampler {sampler}")
+    with pytest.raises(gdrr.GdrrError) as e:
+        gdrr.gdrr_set_spectrum(gdrr.gdrr_create_context(0), np.ones(513) / 513, np.ones(513), np.ones((1, 513)))
+    assert e.value.code == gdrr.GDRR_ERR_INVALID_ARG
+
+
 def test_rays_parallel_to_axes_and_all_miss(gdrr):
     """Odd detector: the central ray is exactly axis parallel at phi = 0 and has
     a zero direction component (reading Q17); a far-off detector misses the box."""
