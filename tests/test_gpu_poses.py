@@ -135,6 +135,29 @@ def test_pose_edge_cases(gdrr):
             pr.project()
 
 
+@pytest.mark.parametrize("sampler", [1, 2])
+def test_skewed_and_stretched_detector_frames(gdrr, workloads_cache, sampler):
+    """u_hat and v_hat are used as given: a frame that is neither unit nor orthogonal (pixels 1.25 x wider along u, v
+    leaning 12 degrees towards u) and a detector rotated in its own plane.  The staged sampler's bound on how far a
+    tile's rays leave the hull of its corner rays scales with these vectors (gdrr_api.cu hull_margins): a wrong bound
+    would show as quads read outside the staged box."""
+    w0 = workloads_cache("C1")
+    phis = np.radians([5.0, 95.0, 230.0])
+    poses = trajectories.circular_poses(w0.sad, w0.sdd, 0.0, phis)
+    skew = poses.copy()
+    skew[:, 6:9] *= 1.25                                                   # stretched u
+    skew[:, 9:12] = np.cos(0.21) * poses[:, 9:12] + np.sin(0.21) * poses[:, 6:9]   # v leaning towards u
+    c, s_ = math.cos(0.6), math.sin(0.6)
+    rot = poses.copy()
+    rot[:, 6:9] = c * poses[:, 6:9] + s_ * poses[:, 9:12]                 # detector rotated by 34 degrees in its plane
+    rot[:, 9:12] = -s_ * poses[:, 6:9] + c * poses[:, 9:12]
+    for what, ps in (("skewed", skew), ("rotated", rot)):
+        w = w0.with_poses(ps)
+        with gdrr.Projector(w, sampler=sampler) as pr:
+            stats = compare_full(pr, w, oracle.project(w), f"{what} frame sampler {sampler}")
+        print(what, sampler, stats)
+
+
 def test_pose_argument_errors(gdrr):
     ctx = gdrr.gdrr_create_context(0)
     try:
