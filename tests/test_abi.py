@@ -35,6 +35,19 @@ def test_library_exports_every_declared_function_and_binding_binds_them():
     assert re.fullmatch(r"\d+\.\d+", g.gdrr_version())
 
 
+def test_header_is_plain_c(tmp_path):
+    """include/gdrr.h is a C header: it compiles alone as C99 (and as C++), no CUDA header needed."""
+    import shutil
+    import subprocess
+    src = tmp_path / "t.c"
+    src.write_text('#include "gdrr.h"\nint main(void) { const char* (*f)(void) = gdrr_version; (void)f; return 0; }\n')
+    inc = os.path.join(ROOT, "include")
+    subprocess.run([shutil.which("gcc") or "gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-fsyntax-only", "-I", inc,
+                    str(src)], check=True)
+    subprocess.run([shutil.which("g++") or "g++", "-std=c++17", "-Wall", "-Werror", "-fsyntax-only", "-x", "c++", "-I", inc,
+                    str(src)], check=True)
+
+
 def test_host_only_calls_return_status_codes():
     import paper_1204_6367_b200 as g
     # workspace sizes are host arithmetic: 16 B per quad for the packed layout, VW floats per padded voxel otherwise
