@@ -239,7 +239,8 @@ GDRR_API int gdrr_project(gdrr_context* ctx, const gdrr_volume* vol, int proj_be
  * caller's device scratch `signal_stage_dev` (>= min(proj_count, stage_proj) *
  * nv*nu floats, stage_proj >= 1 projections per batch) and copies each batch to
  * `signal_host` [proj_count][nv][nu]; returns after the last copy completed.
- * For overlap signal_host should be pinned.  At most four materials (UNSUPPORTED otherwise). */
+ * For overlap signal_host should be pinned.  With more than four materials the line integrals of a batch wait in a
+ * context-owned device scratch (min(proj_count, batch) x n_materials x nv x nu floats, allocated on first use). */
 GDRR_API int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
                       int proj_count, float* signal_host, float* signal_stage_dev,
                       int stage_proj, void* cuda_stream);

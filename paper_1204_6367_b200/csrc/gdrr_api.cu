@@ -40,6 +40,8 @@ struct gdrr_context {
     float* bt_dev = nullptr;
     float* flu_dev = nullptr;
     float* gain_dev = nullptr;      // [n_energy][nv][nu] response gain (gdrr_set_response_gain) or nullptr
+    float* li_scratch = nullptr;    // gdrr_project_host with more than four materials: line integrals of one batch
+    size_t li_scratch_floats = 0;
     // misc
     // pinned, mapped: an ingest kernel sets its volume's slot through flag_dev if it meets a bad material; the slots
     // are handed out round-robin (a slot is reused after kFlagSlots later volumes)
@@ -538,6 +540,7 @@ int gdrr_destroy_context(gdrr_context* ctx) {
     DeviceGuard guard(ctx->device);
     free_dev(ctx->poses_dev); free_dev(ctx->mu_dev); free_dev(ctx->src_dev);
     free_dev(ctx->bt_dev); free_dev(ctx->flu_dev); free_dev(ctx->gain_dev); free_dev(ctx->mu_all_dev);
+    free_dev(ctx->li_scratch);
     if (ctx->flag_host) { cudaFreeHost(ctx->flag_host); ctx->flag_host = nullptr; ctx->flag_dev = nullptr; }
     for (int k = 0; k < 2; ++k) {
         if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
@@ -955,13 +958,24 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
     ProjectParams P;
     int rc = fill_project(ctx, vol, proj_begin, proj_count, P);
     if (rc) return rc;
-    if (!vol->groups.empty())
-        return fail(ctx, GDRR_ERR_UNSUPPORTED, "gdrr_project_host holds at most four materials (no scratch for the line "
-                    "integrals of the groups): use gdrr_project with line_integrals_dev");
     DeviceGuard guard(ctx->device);
     if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSuccess;
+    if (!vol->groups.empty()) {
+        // more than four materials: the groups' line integrals of one batch wait in a context-owned scratch for the
+        // energy sum (the caller gave none); all batches run on stream s, so one scratch serves them in turn
+        const size_t need = (size_t)std::min(proj_count, std::max(1, stage_proj / (stage_proj >= 2 ? 2 : 1))) *
+                            (size_t)vol->n_mat * ctx->nu * ctx->nv;
+        if (ctx->li_scratch_floats < need) {
+            e = cudaStreamSynchronize(s);               // (an earlier call's batches may still read the old one)
+            free_dev(ctx->li_scratch);
+            ctx->li_scratch_floats = 0;
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->li_scratch, sizeof(float) * need);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMalloc(line-integral scratch)");
+            ctx->li_scratch_floats = need;
+        }
+    }
     if (!ctx->copy_stream) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
         if (!ctx->ev_done[k]) e = cudaEventCreateWithFlags(&ctx->ev_done[k], cudaEventDisableTiming);
@@ -983,7 +997,7 @@ int gdrr_project_host(gdrr_context* ctx, const gdrr_volume* vol, int proj_begin,
         ProjectParams Pb = P;
         Pb.g.proj_begin = proj_begin + done;
         Pb.g.proj_count = cnt;
-        Pb.signal = stage; Pb.li = nullptr; Pb.ray_table = nullptr;
+        Pb.signal = stage; Pb.li = vol->groups.empty() ? nullptr : ctx->li_scratch; Pb.ray_table = nullptr;
         e = launch_project(Pb, vol, s);
         if (e != cudaSuccess) break;
         ctx->launches += 1;
