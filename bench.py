@@ -210,6 +210,9 @@ def run_reference(args):
         return
     from workloads import make_workload
     w = make_workload(args.workload, phantom=args.phantom)
+    if args.tissue_classes != 4:
+        from workloads import with_tissue_classes
+        w = with_tissue_classes(w, args.tissue_classes)
     pix, sample = sized_oracle_sample(w, args.ref_seconds)
     for _ in range(args.warmup):
         time_oracle(w, pix[: max(1, len(pix) // 16)])
@@ -254,6 +257,9 @@ def run_b200(args):
 
     # the N-GPU job is one scan of n_proj * N evenly spaced angles, sharded by projection
     w0 = make_workload(args.workload, phantom=args.phantom)
+    if args.tissue_classes != 4:                            # more than four materials: groups of four (include/gdrr.h)
+        from workloads import with_tissue_classes
+        w0 = with_tissue_classes(w0, args.tissue_classes)
     per_gpu = w0.n_proj if args.projections <= 0 else args.projections
     n_total = per_gpu * world
     mine = gd.strided_shard(n_total, world, rank)
@@ -279,6 +285,9 @@ def run_b200(args):
                      sampler={"auto": g.GDRR_SAMPLER_AUTO, "gather": g.GDRR_SAMPLER_GATHER,
                               "staged": g.GDRR_SAMPLER_STAGED}[args.sampler])
     signal = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32, device=dev)
+    # (more than four materials: the library needs the line-integral output, one launch_proj batch of it)
+    li_buf = (torch.empty((min(per_gpu, launch_proj), w.n_materials, w.nv, w.nu), dtype=torch.float32, device=dev)
+              if w.n_materials > 4 else None)
     stream = torch.cuda.current_stream()
     if args.method == "siddon":                            # units = voxel segments of positive length
         n_samples = sum(int(pr.siddon_segments(b, min(32, per_gpu - b)).sum().item()) for b in range(0, per_gpu, 32))
@@ -301,7 +310,7 @@ def run_b200(args):
             events[0].record(stream)
         for b in range(0, per_gpu, launch_proj):            # a1-a7
             cnt = min(launch_proj, per_gpu - b)
-            g.gdrr_project(pr.ctx, pr.vol, b, cnt, signal[b:b + cnt])
+            g.gdrr_project(pr.ctx, pr.vol, b, cnt, signal[b:b + cnt], None if li_buf is None else li_buf[:cnt])
         if events is not None:
             events[1].record(stream)
 
@@ -388,7 +397,7 @@ def run_b200(args):
     l1_achieved = l1_bytes / (kernel_ms * 1e-3) / 1e9
     # what only ncu can see comes from the committed capture of these very sources, or is None (never a stale constant)
     ncu = ncu_constants(kname, args.workload if args.phantom == "smooth" and args.trajectory == "circle"
-                        and not args.u_off_mm else "-")
+                        and not args.u_off_mm and w.n_materials <= 4 else "-")
     dram_step = ncu["dram_bytes_per_projection"] * per_gpu if ncu["dram_bytes_per_projection"] else None
     # the least a projection must move: every voxel of its cone once as a 4-byte word, and its image
     hbm_min = None
@@ -434,6 +443,7 @@ def run_b200(args):
             "data": "synthetic (seeded phantom; DESIGN.md 'Input recipe')",
             "config": dict(workload_config(w, args.workload, world, n_total, launch_proj),
                            phantom=args.phantom, pure_cell_fraction=pure_cell_fraction(w.mat), u_off_mm=w.u_off,
+                           tissue_classes=w.n_materials,
                            inputs_sha256=w.sha256(),
                            **({} if args.trajectory == "circle" else {"trajectory": args.trajectory})),
             "projections_per_s": proj_per_s, "samples_per_step": total_samples,
@@ -544,6 +554,9 @@ def main():
     ap.add_argument("--phantom", default="smooth", choices=["smooth", "noisy1", "noisy3", "random"],
                     help="C2..C4: the BASELINE recipe (smooth), the same with 1 % / 3 % voxel noise before the material "
                          "thresholds, or materials drawn per voxel (workloads/configs.py); the pure-cell fraction is printed")
+    ap.add_argument("--tissue-classes", type=int, default=4, choices=[4, 5, 6, 7, 8],
+                    help="C2..C4 segmented into this many materials (workloads.with_tissue_classes); beyond four the library "
+                         "samples one group of four materials per pass")
     ap.add_argument("--layout", type=int, default=2, help="0 brick (exact), 1 linear (exact), 2 packed quad")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

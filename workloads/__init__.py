@@ -12,7 +12,7 @@ analytic curves stand in for them with the same shapes (SURVEY.md section 8(d),
 DESIGN.md "Input recipe").
 """
 from .prng import SplitMix64
-from .configs import Workload, make_workload, WORKLOAD_NAMES, PHANTOMS, pure_cell_fraction, shard_projections
+from .configs import Workload, make_workload, WORKLOAD_NAMES, PHANTOMS, pure_cell_fraction, with_tissue_classes, shard_projections
 
-__all__ = ["SplitMix64", "Workload", "make_workload", "WORKLOAD_NAMES", "PHANTOMS", "pure_cell_fraction",
+__all__ = ["SplitMix64", "Workload", "make_workload", "WORKLOAD_NAMES", "PHANTOMS", "pure_cell_fraction", "with_tissue_classes",
            "shard_projections"]

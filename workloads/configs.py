@@ -280,6 +280,27 @@ def _volume_pelvis(rng, dims, spacing, phantom="smooth", seed=0):
     return rho, mat, spacing, 4
 
 
+def with_tissue_classes(w, n_classes):
+    """The same volume segmented into `n_classes` materials (5..8) instead of four: density edges at 0.2 (air), 0.98
+    (fat), then tissue and bone split further.  The mass attenuation curves of the new classes are those of the class
+    they were split from, scaled by a few per cent (a seeded stand-in: only the count of materials matters here)."""
+    import copy
+    if not 5 <= n_classes <= 8 or w.n_materials != 4:
+        raise ValueError("with_tissue_classes: 5..8 classes of a four-material workload")
+    edges_all = [0.2, 0.98, 1.03, 1.15, 1.35, 1.6, 1.75]           # 8 classes
+    parent_all = [0, 1, 2, 2, 3, 3, 3, 3]
+    keep = {5: [0, 1, 2, 3], 6: [0, 1, 2, 3, 4], 7: [0, 1, 2, 3, 4, 5], 8: [0, 1, 2, 3, 4, 5, 6]}[n_classes]
+    edges = np.array([edges_all[k] for k in keep], dtype=np.float32)
+    parents = [0] + [parent_all[k + 1] for k in keep]
+    out = copy.copy(w)
+    out.mat = np.digitize(w.rho, edges).astype(np.uint8)
+    out.n_materials = n_classes
+    rng = SplitMix64(BASE_SEED + 77 + n_classes)
+    out.mu_hat = np.ascontiguousarray(np.stack([w.mu_hat[p] * rng.uniform(0.97, 1.03) for p in parents]))
+    out.notes = dict(w.notes, tissue_classes=n_classes)
+    return out
+
+
 def pure_cell_fraction(mat):
     """Fraction of the (nx-1)(ny-1)(nz-1) cells of the voxel lattice whose 8 corner voxels have one material
     (an input statistic: the CUDA sampler's fast path needs such cells)."""
