@@ -74,24 +74,33 @@ __device__ __forceinline__ void finish_pixel(const ProjectParams& P, const float
             if (m < P.n_mat) o[m * plane] = li[m];
     }
     if (P.li_only) return;          // one group of more than four materials: gdrr_energy_sum_kernel forms the signal
-    const float tb = P.bt_thick ? P.bt_thick[i] : 0.f;
-    // pixel-dependent detector response r(E, u) = r(E) g(E, u) (reading Q32): g streams in from global
-    // memory, energy-major, so that the pixels of a warp read neighbouring words
-    const size_t gain_plane = (size_t)P.g.nv * P.g.nu;
-    const float* gain = P.gain ? P.gain + (size_t)j * P.g.nu + i : nullptr;
+    // exp(-tau) as ex2 of the NEGATED optical depth, formed directly: the signs go into the line integrals once
+    const float ntb = P.bt_thick ? -P.bt_thick[i] : 0.f;
+    float nli[VW];
+#pragma unroll
+    for (int m = 0; m < VW; ++m) nli[m] = -li[m];
     float sig = 0.f;
-    for (int e = 0; e < P.n_energy; ++e) {
+    auto bin = [&](int e, float weight) {
         const float4 mu = s_mu[e];
-        float2 sc = s_src[e];
-        if (gain) sc.x *= __ldg(gain + (size_t)e * gain_plane);
-        float tau = sc.y * tb;
-        tau = fmaf(mu.x, li[0], tau);
-        if (VW > 1) tau = fmaf(mu.y, li[VW > 1 ? 1 : 0], tau);
+        float ntau = s_src[e].y * ntb;
+        ntau = fmaf(mu.x, nli[0], ntau);
+        if (VW > 1) ntau = fmaf(mu.y, nli[VW > 1 ? 1 : 0], ntau);
         if (VW > 2) {
-            tau = fmaf(mu.z, li[VW > 2 ? 2 : 0], tau);
-            tau = fmaf(mu.w, li[VW > 2 ? 3 : 0], tau);
+            ntau = fmaf(mu.z, nli[VW > 2 ? 2 : 0], ntau);
+            ntau = fmaf(mu.w, nli[VW > 2 ? 3 : 0], ntau);
         }
-        sig = fmaf(sc.x, exp2f(-tau), sig);
+        sig = fmaf(weight, exp2f(ntau), sig);
+    };
+    if (P.gain) {
+        // pixel-dependent detector response r(E, u) = r(E) g(E, u) (reading Q32): g streams in from global
+        // memory, energy-major, so that the pixels of a warp read neighbouring words.  (Its own loop: predicated off, the
+        // loads and their address arithmetic would still issue in every bin of the common case.)
+        const size_t gain_plane = (size_t)P.g.nv * P.g.nu;
+        const float* gain = P.gain + (size_t)j * P.g.nu + i;
+#pragma unroll 1        // (the rare path: kept small, so that it does not raise the kernels' register counts)
+        for (int e = 0; e < P.n_energy; ++e) bin(e, s_src[e].x * __ldg(gain + (size_t)e * gain_plane));
+    } else {
+        for (int e = 0; e < P.n_energy; ++e) bin(e, s_src[e].x);
     }
     if (P.fluence) sig *= P.fluence[(size_t)j * P.g.nu + i];
     P.signal[((size_t)pl * P.g.nv + j) * P.g.nu + i] = sig;
