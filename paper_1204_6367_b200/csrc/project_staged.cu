@@ -159,10 +159,8 @@ __device__ __forceinline__ void run_chunk_staged_pairs(const Sampler& S, int qx,
             A.cur += blend_cell(a0, c0, fx0, fy0, fz0);
             A.cur += blend_cell(a1, c1, fx1, fy1, fz1);
         } else {
-            // (one more vote per sample: in a noisy volume most failed pairs have one sample that every lane can still
-            // take on the fast path)
-            blend_sample<VW, true>(a0, c0, fx0, fy0, fz0, A);
-            blend_sample<VW, true>(a1, c1, fx1, fy1, fz1, A);
+            blend_sample<VW, false>(a0, c0, fx0, fy0, fz0, A);
+            blend_sample<VW, false>(a1, c1, fx1, fy1, fz1, A);
         }
     }
 }
