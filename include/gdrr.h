@@ -159,8 +159,12 @@ GDRR_API int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host,
                             void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
                             gdrr_volume** out);
 
-/* Waits for the volume's ingest and returns its verdict: OK, INVALID_ARG (a material index >= n_materials was met),
- * CUDA.  The only call on a volume that blocks the host. */
+/* Waits for the volume's ingest (and for the Siddon walk's compact copy, if a Siddon projection of this volume has
+ * been queued) and returns the verdict: OK, INVALID_ARG (a material index >= n_materials was met), CUDA.  The only
+ * call on a volume that blocks the host.  After it has returned OK, gdrr_project on this volume makes no stream call
+ * but its kernel launches on cuda_stream (no event is waited for or queried), so it may be issued inside CUDA stream
+ * capture and replayed as a graph into the same output buffers (tests/test_gpu_graph.py).  For GDRR_METHOD_SIDDON on a
+ * PACKED_QUAD volume, project once before this call: the first Siddon projection makes the compact copy. */
 GDRR_API int gdrr_volume_status(gdrr_context* ctx, const gdrr_volume* vol);
 
 /* Frees the handle, never the workspace. */

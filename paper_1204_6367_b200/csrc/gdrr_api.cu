@@ -78,6 +78,7 @@ struct gdrr_volume {
     std::mutex compact_mu;
     bool compact_launched = false;
     cudaEvent_t compact_done = nullptr;
+    std::atomic<bool> compact_ready{false};   // the copy is known to have finished (gdrr_volume_status): no wait needed
     bool has_tmap = false;      // PACKED_QUAD: tensor map for the staged sampler
     // the device-side material check is read when the ingest has finished, never waited for (volume_check)
     cudaEvent_t ingest_done = nullptr;
@@ -345,6 +346,7 @@ bool make_tensor_map(gdrr_volume* v) {
 cudaError_t ensure_compact(const gdrr_volume* cvol, cudaStream_t s) {
     if (cvol->layout != GDRR_LAYOUT_PACKED_QUAD) return cudaSuccess;
     gdrr_volume* vol = const_cast<gdrr_volume*>(cvol);       // the copy is a cache behind the handle, guarded by its mutex
+    if (vol->compact_ready) return cudaSuccess;              // (no stream call at all: the launch can be captured)
     std::lock_guard<std::mutex> lock(vol->compact_mu);
     cudaError_t e = cudaSuccess;
     if (!vol->compact_launched) {
@@ -742,7 +744,20 @@ int gdrr_create_volume_host(gdrr_context* ctx, const float* rho_host, const uint
 int gdrr_volume_status(gdrr_context* ctx, const gdrr_volume* vol) {
     if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
     if (!vol || vol->ctx != ctx) return fail(ctx, GDRR_ERR_INVALID_ARG, "volume is NULL or belongs to another context");
-    return volume_check(ctx, vol, true);
+    if (int rc = volume_check(ctx, vol, true)) return rc;
+    // also the Siddon walk's compact copy, where one has been launched: after this call nothing the library enqueues
+    // for this volume waits on an event, which is what stream capture needs (tests/test_gpu_graph.py)
+    for (size_t g = 0; g <= vol->groups.size(); ++g) {
+        gdrr_volume* member = const_cast<gdrr_volume*>(g == 0 ? vol : vol->groups[g - 1]);
+        std::lock_guard<std::mutex> lock(member->compact_mu);
+        if (member->compact_launched && !member->compact_ready) {
+            DeviceGuard guard(ctx->device);
+            if (cudaError_t e = cudaEventSynchronize(member->compact_done))
+                return cuda_fail(ctx, e, "waiting for the compact copy");
+            member->compact_ready = true;
+        }
+    }
+    return GDRR_OK;
 }
 
 int gdrr_destroy_volume(gdrr_volume* vol) {
