@@ -95,16 +95,18 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def source_digest():
-    """sha256 over the DEVICE sources (every file of csrc/ but the host-side gdrr_api.cu): the stamp that ties
-    profiles/ncu_constants.json to the kernels it was captured on."""
+def source_digest(files=None):
+    """sha256 over device sources of csrc/: the stamp that ties a record of profiles/ncu_constants.json to the kernel it
+    was captured on.  `files`: the kernel's own translation unit, the headers it includes and the ingest that lays out
+    the volume it reads (the record lists them); None = every file but the host-side gdrr_api.cu."""
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_1204_6367_b200", "csrc")
-    for name in sorted(os.listdir(csrc)):
-        if name.endswith((".cu", ".cuh", ".h")) and name != "gdrr_api.cu":
-            with open(os.path.join(csrc, name), "rb") as f:
-                h.update(name.encode() + b"\0" + f.read())
+    if files is None:
+        files = [n for n in os.listdir(csrc) if n.endswith((".cu", ".cuh", ".h")) and n != "gdrr_api.cu"]
+    for name in sorted(files):
+        with open(os.path.join(csrc, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
     return h.hexdigest()
 
 
@@ -123,7 +125,12 @@ def ncu_constants(kernel, workload):
     if rec is None:
         return none
     rec = dict(rec)
-    rec["matches_this_build"] = table.get("source_sha256") == source_digest()
+    # (a record stamped with its own source list is valid while THOSE files are unchanged; older records carry the
+    # digest of all device sources)
+    if "sources" in rec:
+        rec["matches_this_build"] = rec.get("source_sha256") == source_digest(rec["sources"])
+    else:
+        rec["matches_this_build"] = table.get("source_sha256") == source_digest()
     if not rec["matches_this_build"]:
         for k in ("dram_bytes_per_projection", "l2_to_sm_bytes_per_sample", "bound_busy_frac"):
             rec[k] = None

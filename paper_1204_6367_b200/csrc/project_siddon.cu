@@ -5,11 +5,15 @@
 // One thread per detector pixel.  Ray setup in fp64 (ray_setup.cuh, the same clip of the
 // source->pixel segment to the volume box as the tri-linear method).  The traversal is the
 // incremental form of Siddon's merge: per axis the parameter of the next lattice plane the
-// ray meets, the smallest of the three ends the current voxel's segment.  Parameters are
-// kept in fp32 RELATIVE TO THE ENTRY POINT (range 0 .. chord, <= a few hundred mm) and are
-// formed as fma(plane counter, dt, t0) from integer counters, never by repeated addition, so a
-// crossing is placed within one ulp of the chord (3e-5 mm at 500 mm) however long the ray;
-// a boundary misplaced by that much changes LI by 3e-5 mm x the density jump (~1e-7 relative).
+// ray meets, the smallest of the three ends the current voxel's segment.  The walk runs in
+// chunks of 32 steps on fp32 parameters LOCAL to the chunk (relative to a point near the entry
+// of its first voxel, so below ~50 mm); at every chunk start they are formed anew IN FP64
+// from the count of planes crossed, count x dt + t0 minus that point, with the ray's fp64
+// constants read back from shared memory.  A crossing is then placed within the 32 fp32
+// additions of one chunk (<= 6e-5 mm, typically 5e-6) however long the ray.  (Round 2's first
+// form rounded count x dt + t0 to fp32 at the chord's magnitude: 3e-5 mm per plane plus the
+// rounding of dt times the count, 1.2e-4 mm between two axes; behind a bone / air jump that
+// is 4e-4 mm g/cm^3, which the whole-scan parity run met once in 48 projections of C3.)
 // Segments of zero or negative length (ties at lattice edges, rounding) contribute nothing.
 //
 // Works on every device layout: the exact ones hold VW floats per voxel (one per material),
@@ -49,6 +53,13 @@ __device__ __forceinline__ int siddon_axis_offset(int i, int stride) {
     return i * stride;
 }
 
+// fp64 -> fp32 as one F2F (under -ftz the plain cast adds a compare and a multiply to flush denormals, which never occur here)
+__device__ __forceinline__ float to_float(double x) {
+    float f;
+    asm("cvt.rn.f32.f64 %0, %1;" : "=f"(f) : "d"(x));
+    return f;
+}
+
 // The material of the walk changes (a few times per ray): the closed run goes to its material's slot.  Out of line, so
 // that the walk's loop keeps a plain branch around it instead of ten predicated instructions in every step.
 __device__ __noinline__ void route_out_of_line(float* slot, unsigned m, float v) { slot[m * kAccStride] += v; }
@@ -66,10 +77,13 @@ __device__ __forceinline__ typename SiddonVoxel<VW, LAYOUT>::T load_voxel(const 
 // LAYOUT: 0 brick, 1 linear (exact, VW floats per voxel), 2 packed volume's compact copy (one word per voxel)
 // COUNT: also count the segments of positive length (gdrr_siddon_segments)
 template <int VW, int LAYOUT, bool COUNT>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 5)           // 48 registers: 5 CTAs per SM (4 at the 54 ptxas takes if left alone)
 gdrr_project_siddon_kernel(const ProjectParams P) {
     using VT = typename SiddonVoxel<VW, LAYOUT>::T;
     __shared__ float s_acc[LAYOUT == 2 ? 4 : 1][LAYOUT == 2 ? kAccStride : 1];      // per-material sums of a packed walk
+    __shared__ double s_ray[7][kThreads];           // this thread's t0[3], dt[3], t_end in fp64 (read at chunk starts only)
+    __shared__ float s_idt[3][kThreads];            // ... 1 / dt (0 for an axis the ray does not move along)
+    __shared__ float s_t0[3][kThreads];             // ... and t0 rounded to fp32, for the plane counts
     float4* s_mu;
     float2* s_src;
     load_tables(P, s_mu, s_src);
@@ -100,25 +114,29 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
             int v = (int)floor((x - P.g.lo[a]) / P.g.d[a]);
             v = min(max(v, 0), N - 1);
             idx[a] = v;
+            double t0d = 3.0e38, dtd = 0.0;
             if (r.dir[a] > 0.0) {
                 stp[a] = 1;
-                t0[a] = (float)((P.g.lo[a] + (double)(v + 1) * P.g.d[a] - r.S[a]) / r.dir[a] - r.t_in);
-                dt[a] = (float)(P.g.d[a] / r.dir[a]);
+                t0d = (P.g.lo[a] + (double)(v + 1) * P.g.d[a] - r.S[a]) / r.dir[a] - r.t_in;
+                dtd = P.g.d[a] / r.dir[a];
             } else if (r.dir[a] < 0.0) {
                 stp[a] = -1;
-                t0[a] = (float)((P.g.lo[a] + (double)v * P.g.d[a] - r.S[a]) / r.dir[a] - r.t_in);
-                dt[a] = (float)(-P.g.d[a] / r.dir[a]);
+                t0d = (P.g.lo[a] + (double)v * P.g.d[a] - r.S[a]) / r.dir[a] - r.t_in;
+                dtd = -P.g.d[a] / r.dir[a];
             } else {
                 stp[a] = 0;
-                t0[a] = 3.0e38f;
-                dt[a] = 0.f;
             }
+            t0[a] = (float)t0d;
+            dt[a] = (float)dtd;
+            s_ray[a][threadIdx.x] = t0d;
+            s_ray[3 + a][threadIdx.x] = dtd;
+            s_t0[a][threadIdx.x] = t0[a];
+            s_idt[a][threadIdx.x] = dt[a] > 0.f ? 1.f / dt[a] : 0.f;     // (0: that axis' parameter stays 3e38)
         }
-        const float t_end = (float)(r.t_out - r.t_in);
-        // The plane through which the ray leaves the box has the parameter t_end up to ~3 ulp (t0, dt and
-        // t_end are rounded separately): a crossing within 16 ulp of the end IS the end, so the walk never
-        // steps out of the lattice; the sliver it may drop is < 5e-4 mm of the last voxel.
-        const float t_stop = t_end * (1.f - 16.f * 5.96e-8f);
+        s_ray[6][threadIdx.x] = r.t_out - r.t_in;
+        // The plane through which the ray leaves the box has the chunk-local parameter te up to the fp32 additions of
+        // one chunk (<= 32 x half an ulp of te): a crossing within 64 ulp of the end IS the end, so the walk never
+        // steps out of the lattice; the sliver it may drop is < 4e-6 of the last chunk's length (2e-4 mm at 50 mm).
         constexpr int sx = (LAYOUT == 0) ? 8 : 1;
         const int sy = LAYOUT == 2 ? P.v.cstride_y : P.v.stride_y, sz = LAYOUT == 2 ? P.v.cstride_z : P.v.stride_z;
         const void* vox = LAYOUT == 2 ? P.v.compact : P.v.vox;
@@ -127,18 +145,16 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
         // linear element orders: stepping one voxel along an axis adds a constant to the element offset
         const int dox = stp[0] * (LAYOUT == 2 ? 4 : sx), doy = stp[1] * sy, doz = stp[2] * sz;
         const int y_edge = stp[1] > 0 ? 3 : 0, doy_cross = stp[1] * (sy - 3);       // LAYOUT 2 only
-        // 1 / dt for the re-base (0 for an axis the ray does not move along: its parameter stays 3e38)
-        const float idt[3] = {dt[0] > 0.f ? 1.f / dt[0] : 0.f, dt[1] > 0.f ? 1.f / dt[1] : 0.f,
-                              dt[2] > 0.f ? 1.f / dt[2] : 0.f};
         // Inside a chunk of kMaxChunk steps the parameters are LOCAL: relative to the point where the chunk's first voxel
         // was entered (tg, a parameter relative to the ray's entry), so that they stay below ~50 mm and the one addition
         // of dt per step costs 32 x half an ulp of THAT (6e-5 mm) instead of the chord's (5e-4 mm at 500 mm: measured
         // as 1.2e-3 of LI error behind a density jump on C2).  At a chunk's start the three global parameters are formed
-        // anew as fma(planes crossed, dt, t0) -- the count is what the drifted value still gives when rounded -- so
-        // nothing accumulates from chunk to chunk.
-        float tg = 0.f;
+        // anew in fp64 as fma(planes crossed, dt, t0) -- the count is what the drifted fp32 value still gives when
+        // rounded -- and the frame's origin is taken off in fp64 too, so nothing accumulates from chunk to chunk and
+        // nothing is rounded at the chord's magnitude.
+        float tg = 0.f, t = 0.f;
         float tx = t0[0], ty = t0[1], tz = t0[2];
-        float te = t_end, ts = t_stop;
+        float te = 0.f, ts = 0.f;
         RayAcc<VW> A;                                    // LAYOUT 2: running sum of the current material (packed_sampler.cuh)
         if (LAYOUT == 2) init_ray<VW>(A, &s_acc[0][threadIdx.x]);
 
@@ -157,16 +173,25 @@ gdrr_project_siddon_kernel(const ProjectParams P) {
 #pragma unroll
             for (int m = 0; m < VW; ++m) part[m] = 0.f;
             {
-                const float gx = fmaf(rintf((tg + tx - t0[0]) * idt[0]), dt[0], t0[0]);
-                const float gy = fmaf(rintf((tg + ty - t0[1]) * idt[1]), dt[1], t0[1]);
-                const float gz = fmaf(rintf((tg + tz - t0[2]) * idt[2]), dt[2], t0[2]);
-                // the current voxel was entered at the last plane crossed (an axis the ray does not move along has none)
-                tg = fmaxf(fmaxf(dt[0] > 0.f ? gx - dt[0] : 0.f, dt[1] > 0.f ? gy - dt[1] : 0.f),
-                           fmaxf(dt[2] > 0.f ? gz - dt[2] : 0.f, 0.f));
-                tx = gx - tg; ty = gy - tg; tz = gz - tg;
-                te = t_end - tg; ts = t_stop - tg;
+                // origin of the chunk's frame: the fp32 sum below, taken as exact (any point near the entry of the
+                // current voxel serves; what matters is that every parameter is taken relative to the SAME number)
+                const float ref = tg + t;
+                const double refd = (double)ref;
+                const double gx = fma((double)rintf((tg + tx - s_t0[0][threadIdx.x]) * s_idt[0][threadIdx.x]),
+                                      s_ray[3][threadIdx.x], s_ray[0][threadIdx.x]);
+                const double gy = fma((double)rintf((tg + ty - s_t0[1][threadIdx.x]) * s_idt[1][threadIdx.x]),
+                                      s_ray[4][threadIdx.x], s_ray[1][threadIdx.x]);
+                const double gz = fma((double)rintf((tg + tz - s_t0[2][threadIdx.x]) * s_idt[2][threadIdx.x]),
+                                      s_ray[5][threadIdx.x], s_ray[2][threadIdx.x]);
+                tx = to_float(gx - refd); ty = to_float(gy - refd); tz = to_float(gz - refd);
+                te = to_float(s_ray[6][threadIdx.x] - refd);
+                ts = te * (1.f - 64.f * 5.96e-8f);
+                tg = ref;
+                // the current voxel was entered at the last plane crossed (an axis the ray does not move along has none;
+                // the ray's own entry is 0 - ref): local magnitudes, so fp32 places it within 1e-6 mm
+                t = fmaxf(fmaxf(dt[0] > 0.f ? tx - dt[0] : -ref, dt[1] > 0.f ? ty - dt[1] : -ref),
+                          fmaxf(dt[2] > 0.f ? tz - dt[2] : -ref, -ref));
             }
-            float t = 0.f;
 #pragma unroll 2
             for (int s = 0; s < kMaxChunk && more; ++s) {
                 const float tn = fminf(fminf(tx, ty), fminf(tz, te));       // where the ray leaves this voxel
