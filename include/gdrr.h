@@ -326,6 +326,23 @@ GDRR_API int gdrr_denoise_scatter(gdrr_context* ctx, const float* s_hat_dev, flo
                          int nu, int nv, int n_images, double beta, double omega, int n_iter,
                          double floor_value, void* cuda_stream);
 
+/* The same sweeps for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no scratch_dev argument, and the call makes no cudaMalloc, cudaFree or allocating
+ * library call.  The scratch image is a static array inside the library: every GPU that loads the library holds
+ * GDRR_DENOISE_STATIC_MAX_FLOATS x 4 bytes (16 MiB) of it until the process exits.
+ *   s_hat_dev, s_dev   as for gdrr_denoise_scatter (the caller's buffers; s_dev receives the result)
+ * Limit: nu * nv * n_images <= GDRR_DENOISE_STATIC_MAX_FLOATS (e.g. 21 images of 512 x 384), else UNSUPPORTED with a
+ * message that names the limit; other errors as gdrr_denoise_scatter.  Results are bit-identical to gdrr_denoise_scatter.
+ * ALL calls, on all contexts and streams of a GPU, share the one array, and it keeps the last call's contents (which
+ * no call reads: every launch writes each pixel of its destination before a later launch reads it, so nothing has to
+ * start at zero).  Calls that overlap on the GPU (different streams, concurrent graph replays) RACE on it: issue them
+ * on one stream, or order them yourself.  The first call on a device resolves the array's address there
+ * (cudaGetSymbolAddress, once per device): make that first call outside stream capture. */
+#define GDRR_DENOISE_STATIC_MAX_FLOATS 4194304
+GDRR_API int gdrr_denoise_scatter_static(gdrr_context* ctx, const float* s_hat_dev, float* s_dev,
+                                int nu, int nv, int n_images, double beta, double omega, int n_iter,
+                                double floor_value, void* cuda_stream);
+
 /* Number of kernels this library has launched on ctx since creation (for the
  * harness's gpu_launches count). */
 GDRR_API unsigned long long gdrr_kernel_launches(const gdrr_context* ctx);

@@ -35,6 +35,7 @@ GDRR_METHOD_SIDDON = 1
 GDRR_METHOD_TEXTURE = 2
 GDRR_MAX_MATERIALS = 16
 GDRR_MAX_ENERGIES = 512
+GDRR_DENOISE_STATIC_MAX_FLOATS = 4194304
 
 EXPORTS = (
     "gdrr_create_context", "gdrr_destroy_context", "gdrr_last_error",
@@ -42,6 +43,7 @@ EXPORTS = (
     "gdrr_destroy_volume", "gdrr_set_geometry", "gdrr_set_spectrum", "gdrr_project",
     "gdrr_project_host", "gdrr_ray_setup", "gdrr_kernel_launches", "gdrr_version",
     "gdrr_set_method", "gdrr_siddon_segments", "gdrr_set_sampler", "gdrr_volume_attach_texture", "gdrr_denoise_scatter",
+    "gdrr_denoise_scatter_static",
     "gdrr_set_geometry_poses", "gdrr_last_sampler", "gdrr_debug_set_skew", "gdrr_debug_ray_cells",
     "gdrr_set_response_gain", "gdrr_volume_status",
 )
@@ -80,6 +82,7 @@ def _load():
         "gdrr_set_sampler": (i, [vp, i]),
         "gdrr_volume_attach_texture": (i, [vp, vp, vp]),
         "gdrr_denoise_scatter": (i, [vp, vp, vp, vp, i, i, i, d, d, i, d, vp]),
+        "gdrr_denoise_scatter_static": (i, [vp, vp, vp, i, i, i, d, d, i, d, vp]),
         "gdrr_siddon_segments": (i, [vp, vp, i, i, vp, vp]),
         "gdrr_set_response_gain": (i, [vp, vp]),
         "gdrr_last_sampler": (i, [vp]),
@@ -329,6 +332,17 @@ def gdrr_denoise_scatter(ctx, s_hat_dev, s_dev, scratch_dev, beta, n_iter, omega
     _check(_lib.gdrr_denoise_scatter(ctx, _dev(s_hat_dev, "float32", n, "s_hat_dev"), _dev(s_dev, "float32", n, "s_dev"),
                                      _dev(scratch_dev, "float32", n, "scratch_dev"), nu, nv, n_images, float(beta),
                                      float(omega), int(n_iter), float(floor_value), _stream(stream)), ctx)
+
+
+def gdrr_denoise_scatter_static(ctx, s_hat_dev, s_dev, beta, n_iter, omega=0.8, floor_value=1e-12, stream=None):
+    """gdrr_denoise_scatter without a scratch tensor: the library's static scratch array (at most
+    GDRR_DENOISE_STATIC_MAX_FLOATS pixels per call; calls that overlap on the GPU race on it)."""
+    shape = tuple(s_hat_dev.shape)
+    n_images, nv, nu = (1,) + shape if len(shape) == 2 else shape
+    n = n_images * nv * nu
+    _check(_lib.gdrr_denoise_scatter_static(ctx, _dev(s_hat_dev, "float32", n, "s_hat_dev"),
+                                            _dev(s_dev, "float32", n, "s_dev"), nu, nv, n_images, float(beta),
+                                            float(omega), int(n_iter), float(floor_value), _stream(stream)), ctx)
 
 
 def gdrr_set_sampler(ctx, sampler):

@@ -8,6 +8,8 @@
 // the cells at least t away from such edges are exact; those include the CTA's output tile.
 // At an image edge the tile ends with the image and clamping the neighbour index to the tile IS
 // the replicated edge.  fp32 arithmetic; S_hat / S by reciprocal and multiply (2 ulp, far inside the tolerance).
+#include <mutex>
+
 #include "gdrr_internal.h"
 
 namespace gdrr {
@@ -106,6 +108,42 @@ cudaError_t launch_denoise(const float* s_hat, float* s_dev, float* scratch, int
         which ^= 1;
     }
     return cudaSuccess;
+}
+
+// ---- gdrr_denoise_scatter_static: the same sweeps for callers that cannot allocate (include/gdrr.h) ----------------
+// The ping-pong scratch image is this file-scope array instead of a caller's buffer.  Every GPU that loads the library
+// holds its kDenoiseStaticFloats x 4 B (16 MiB) from the first use of the module until the process exits.
+// In HOST code the name `g_denoise_scratch` is a host-side stand-in, not a device address: the address the kernel gets
+// is the one cudaGetSymbolAddress returns on the current device, resolved here once per device.
+// Nothing in it has to start at zero: a launch writes every pixel of its destination image before any later launch
+// reads it, and the call's result ends in the caller's s_dev, so the contents a previous call left are never read.
+// All calls share the one array: two calls that overlap on a GPU (different streams, or graphs replayed concurrently) race.
+static __device__ __align__(256) float g_denoise_scratch[kDenoiseStaticFloats];
+
+constexpr int kMaxDevices = 64;
+
+cudaError_t launch_denoise_static(const float* s_hat, float* s_dev, int nu, int nv, int n_images, double beta, double omega,
+                                  int n_iter, double floor_value, cudaStream_t st, int* launches) {
+    static std::mutex mu;
+    static float* addr[kMaxDevices] = {};           // device address of g_denoise_scratch, per device ordinal
+    *launches = 0;
+    if ((size_t)nu * (size_t)nv * (size_t)n_images > kDenoiseStaticFloats) return cudaErrorInvalidValue;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    float* scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (!addr[dev]) {                            // set-up, once per device, with that device current
+            float* p = nullptr;
+            e = cudaGetSymbolAddress((void**)&p, g_denoise_scratch);
+            if (e != cudaSuccess) return e;
+            addr[dev] = p;
+        }
+        scratch = addr[dev];
+    }
+    return launch_denoise(s_hat, s_dev, scratch, nu, nv, n_images, beta, omega, n_iter, floor_value, st, launches);
 }
 
 }  // namespace gdrr

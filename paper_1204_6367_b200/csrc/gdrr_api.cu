@@ -1105,6 +1105,34 @@ int gdrr_denoise_scatter(gdrr_context* ctx, const float* s_hat_dev, float* s_dev
     return GDRR_OK;
 }
 
+static_assert(kDenoiseStaticFloats == (size_t)GDRR_DENOISE_STATIC_MAX_FLOATS, "header and denoise.cu disagree");
+
+// The denoiser for callers that cannot allocate: no cudaMalloc / cudaFree / allocating library call on this path.
+int gdrr_denoise_scatter_static(gdrr_context* ctx, const float* s_hat_dev, float* s_dev, int nu, int nv, int n_images,
+                                double beta, double omega, int n_iter, double floor_value, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
+    if (!s_hat_dev || !s_dev) return fail(ctx, GDRR_ERR_INVALID_ARG, "a device pointer is NULL");
+    if (nu <= 0 || nv <= 0 || n_images <= 0 || n_iter < 0)
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "need positive sizes and n_iter >= 0");
+    if (!(beta > 0.0) || !std::isfinite(beta) || !(floor_value > 0.0) || !(omega > 0.0) || !(omega < 2.0))
+        return fail(ctx, GDRR_ERR_INVALID_ARG, "need beta > 0, floor_value > 0 and 0 < omega < 2");
+    if (n_images > 65535) return fail(ctx, GDRR_ERR_UNSUPPORTED, "at most 65535 images per call");
+    const double pixels = (double)nu * (double)nv * (double)n_images;
+    if (pixels > (double)GDRR_DENOISE_STATIC_MAX_FLOATS)
+        return fail(ctx, GDRR_ERR_UNSUPPORTED,
+                    "%d images of %d x %d = %.0f pixels exceed the static scratch of GDRR_DENOISE_STATIC_MAX_FLOATS = %d "
+                    "pixels; use gdrr_denoise_scatter with a scratch buffer of your own, or fewer images per call",
+                    n_images, nu, nv, pixels, (int)GDRR_DENOISE_STATIC_MAX_FLOATS);
+    DeviceGuard guard(ctx->device);
+    if (guard.status != cudaSuccess) return cuda_fail(ctx, guard.status, "cudaSetDevice");
+    int launches = 0;
+    cudaError_t e = launch_denoise_static(s_hat_dev, s_dev, nu, nv, n_images, beta, omega, n_iter, floor_value,
+                                          (cudaStream_t)cuda_stream, &launches);
+    ctx->launches += launches;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "denoise kernel launch (static scratch)");
+    return GDRR_OK;
+}
+
 int gdrr_set_sampler(gdrr_context* ctx, int sampler) {
     if (!ctx) return fail(nullptr, GDRR_ERR_INVALID_ARG, "ctx is NULL");
     if (sampler != GDRR_SAMPLER_AUTO && sampler != GDRR_SAMPLER_GATHER && sampler != GDRR_SAMPLER_STAGED)
