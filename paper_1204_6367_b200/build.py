@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgdrr_b200.so")
 SOURCES = ["gdrr_api.cu", "project_fused.cu", "project_packed.cu", "project_staged.cu", "project_siddon.cu", "project_texture.cu", "denoise.cu", "volume_layout.cu", "debug_cells.cu", "energy_sum.cu"]
-HEADERS = ["gdrr_internal.h", "ray_setup.cuh", "project_common.cuh", "packed_sampler.cuh", os.path.join(ROOT, "include", "gdrr.h")]
+HEADERS = ["gdrr_internal.h", "denoise_static.h", "ray_setup.cuh", "project_common.cuh", "packed_sampler.cuh", os.path.join(ROOT, "include", "gdrr.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

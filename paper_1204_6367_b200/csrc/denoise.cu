@@ -10,6 +10,7 @@
 // the replicated edge.  fp32 arithmetic; S_hat / S by reciprocal and multiply (2 ulp, far inside the tolerance).
 #include <mutex>
 
+#include "denoise_static.h"
 #include "gdrr_internal.h"
 
 namespace gdrr {

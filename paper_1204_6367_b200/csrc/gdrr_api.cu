@@ -17,6 +17,7 @@
 #include <vector>
 
 #include "../../include/gdrr.h"
+#include "denoise_static.h"
 #include "gdrr_internal.h"
 
 using namespace gdrr;

@@ -111,10 +111,5 @@ cudaError_t launch_ray_setup(const GeomParams& g, int32_t* ray_table,
 cudaError_t launch_energy_sum(const ProjectParams& p, cudaStream_t s);
 cudaError_t launch_denoise(const float* s_hat, float* s_dev, float* scratch, int nu, int nv, int n_images,
                            double beta, double omega, int n_iter, double floor_value, cudaStream_t st, int* launches);
-// the same with the scratch image in a file-scope __device__ array of kDenoiseStaticFloats floats (denoise.cu);
-// = GDRR_DENOISE_STATIC_MAX_FLOATS of include/gdrr.h (gdrr_api.cu asserts it)
-constexpr size_t kDenoiseStaticFloats = (size_t)4 << 20;
-cudaError_t launch_denoise_static(const float* s_hat, float* s_dev, int nu, int nv, int n_images, double beta, double omega,
-                                  int n_iter, double floor_value, cudaStream_t st, int* launches);
 
 }  // namespace gdrr
