@@ -39,6 +39,60 @@ def face_tie_checker(w, projections):
     return near_face
 
 
+SLIVER_MM = 1e-3      # two lattice planes of different axes crossed within this length: their order is a tie (Q26)
+
+
+def siddon_sliver_checker(w, projections, found=None):
+    """near_face(index) for check_line_integrals on Siddon images [P][M][nv][nu] of the circular-gantry workload `w`:
+    True iff the ray of that pixel, in the oracle's own fp64 geometry, crosses two lattice planes of DIFFERENT axes
+    within SLIVER_MM of path length at a lattice edge one of whose four voxels holds the entry's material with
+    rho > 0.  The ray has a sliver of one of those voxels; fp32 can order the two crossings the other way round and
+    then has a sliver of the diagonal neighbour instead (reading Q26: both are valid).  If that voxel is the ray's
+    only piece of the material, its line integral is a non-zero sliver against an exact 0 (or the reverse), below the
+    floor like every other error.  `found`: list that collects the entries asked about."""
+    import oracle
+    rho, mat = np.asarray(w.rho), np.asarray(w.mat)
+    dims = [int(n) for n in w.dims]
+    spacing = [float(d) for d in w.spacing]
+    lo = [float(w.centre[a]) - 0.5 * dims[a] * spacing[a] for a in range(3)]
+
+    def near_edge(index):
+        p, m, j, i = (int(x) for x in index)
+        if found is not None:
+            found.append((int(projections[p]), m, j, i))
+        r = oracle.ray(w, float(w.phis[projections[p]]), i, j)
+        if not r["hit"]:
+            return False
+        S, d = r["S"], r["dir"]
+        unit = float(np.linalg.norm(d))
+        eps = SLIVER_MM / unit
+        ts, ax = [], []
+        for a in range(3):
+            if d[a] == 0.0:
+                continue
+            t = (lo[a] + np.arange(dims[a] + 1) * spacing[a] - S[a]) / d[a]
+            t = t[(t >= r["t_in"] - eps) & (t <= r["t_out"] + eps)]
+            ts.append(t)
+            ax.append(np.full(len(t), a))
+        ts, ax = np.concatenate(ts), np.concatenate(ax)
+        order = np.argsort(ts, kind="stable")
+        ts, ax = ts[order], ax[order]
+        ties = np.nonzero((np.diff(ts) * unit < SLIVER_MM) & (ax[1:] != ax[:-1]))[0]
+        for k in ties:
+            a, b = int(ax[k]), int(ax[k + 1])
+            c = [(S[q] + 0.5 * (ts[k] + ts[k + 1]) * d[q] - lo[q]) / spacing[q] for q in range(3)]
+            third = 3 - a - b
+            for da in (-1, 0):
+                for db in (-1, 0):
+                    v = [0, 0, 0]
+                    v[a], v[b], v[third] = int(round(c[a])) + da, int(round(c[b])) + db, int(np.floor(c[third]))
+                    if all(0 <= v[q] < dims[q] for q in range(3)) \
+                            and int(mat[v[2], v[1], v[0]]) == m and float(rho[v[2], v[1], v[0]]) > 0.0:
+                        return True
+        return False
+    return near_edge
+
+
 def check_line_integrals(li_gpu, li_ref, what="", near_face=None):
     li_gpu = np.asarray(li_gpu, dtype=np.float64)
     li_ref = np.asarray(li_ref, dtype=np.float64)

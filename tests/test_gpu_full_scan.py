@@ -23,7 +23,7 @@ torch = pytest.importorskip("torch")
 
 import oracle  # noqa: E402
 from parity_util import (LI_FLOOR, LI_RTOL, check_line_integrals, check_ray_table, check_signal,  # noqa: E402
-                         face_tie_checker)
+                         face_tie_checker, siddon_sliver_checker)
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -70,9 +70,13 @@ def _scan_parity(gdrr, w, name, projections, block, sampler=0, layout=2, method=
             what = f"{name} projections {idx[0]}..{idx[-1]}"
             check_ray_table(tab, ref["ray_table"], what)
             rec["face_tie_entries"] += int(np.count_nonzero((ref["line_integrals"] == 0.0) & (li != 0.0)))
-            # (the face tie of reading Q9 is a property of the midpoint rule's sample positions: no exception for Siddon)
+            # (the face tie of reading Q9 belongs to the midpoint rule's sample positions; Siddon's walk has the sliver
+            # tie of reading Q26 instead: the ray must be shown to cross two planes within 1e-3 mm of each other)
+            slivers = []
             rel_li, n_floor = check_line_integrals(li, ref["line_integrals"], what,
-                                                   None if siddon else face_tie_checker(w, idx))
+                                                   siddon_sliver_checker(w, idx, slivers) if siddon
+                                                   else face_tie_checker(w, idx))
+            rec["sliver_tie_entries"] = rec.get("sliver_tie_entries", 0) + len(slivers)
             rel_sig = check_signal(sig, ref["signal"], what)
             rec["pixels"] += int(sig.size)
             rec["samples"] += int(ref["ray_table"][..., 1].sum())
@@ -143,6 +147,19 @@ def test_c3_whole_scan_siddon_per_pixel(gdrr, workloads_cache, request):
         _record("C3_siddon", rec)
     else:
         rec = _scan_parity(gdrr, w, "C3", _projection_list(w.n_proj, False, 30), 8, method="siddon")
+    print(json.dumps(rec))
+    assert rec["ray_table_differences"] == 0 and rec["worst_rel_signal"] <= 1e-4
+
+
+def test_c4_whole_scan_siddon_per_pixel(gdrr, workloads_cache, request):
+    """The same on C4: all 656 projections with --full-scan (3.3e11 voxel segments), else every 82nd."""
+    full = request.config.getoption("--full-scan")
+    w = workloads_cache("C4")
+    if full:
+        rec = _scan_parity(gdrr, w, "C4", list(range(w.n_proj)), 4, method="siddon")
+        _record("C4_siddon", rec)
+    else:
+        rec = _scan_parity(gdrr, w, "C4", _projection_list(w.n_proj, False, 82), 4, method="siddon")
     print(json.dumps(rec))
     assert rec["ray_table_differences"] == 0 and rec["worst_rel_signal"] <= 1e-4
 
