@@ -125,22 +125,35 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
 // The same, FOUR consecutive elements of a row per thread, for volumes whose rows are 4-voxel aligned (nx % 4 == 0,
 // aligned input pointers: launch_ingest checks).  The four elements need voxel columns ex0 - 1 .. ex0 + 3 of two rows in
 // two slabs; away from the volume's faces that is one aligned 4-byte word of materials plus one byte, and one float4 of
-// densities plus one float, per row and slab: 12 loads for four elements where the kernel above issues 48, and each
-// voxel's material is mapped once instead of up to four times.  Bit-identical output.
-__global__ void __launch_bounds__(128)
+// densities plus one float, per row and slab: 12 loads for four elements where the kernel above issues 48.  Each
+// voxel's material is mapped once (the kernel above: up to four times), the set of materials of a cell is the OR of two
+// per-COLUMN sets (a column = the 2 x 2 voxels of one x), and the range check looks at the four voxels this thread
+// alone owns (slab ez - 1, row ey - 1, columns ex0 .. ex0 + 3: every voxel has exactly one such owner, and at the
+// faces a few more).  A block is 32 threads (x) by kIngestRows rows: neighbouring rows find each other's voxels in L1
+// (measured on C3, ms per ingest: 2 rows 0.341, 4 rows 0.345, 8 rows 0.355; the round's first form of this kernel 0.529).
+// Bit-identical output (tests/test_gpu_ingest.py).
+constexpr int kIngestRows = 2;
+__global__ void __launch_bounds__(32 * kIngestRows)
 gdrr_ingest_packed4_kernel(const IngestParams P) {
-    const int ez = P.ez0 + blockIdx.z, ey = blockIdx.y;
-    const int ex0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int ez = P.ez0 + blockIdx.z, ey = kIngestRows * blockIdx.y + threadIdx.y;
+    const int ex0 = 4 * (blockIdx.x * 32 + threadIdx.x);
+    if (ey >= P.py) return;
     const int row_slots = (ey == P.py - 1) ? P.sz - ey * P.sy : P.sy;      // the last row also owns the slab's tail pad
     if (ex0 >= row_slots) return;
     uint4 out[4];
 #pragma unroll
     for (int e = 0; e < 4; ++e) out[e] = make_uint4(0u, 0u, 0u, 0u);
-    if (ex0 < P.px && ey < P.py) {
-        unsigned tag[2][2][5];          // [slab][row][column]: material as this device volume's tag
-        unsigned bits[2][5];            // [row][column]: word of slab 0 (rho, tagged)
-        // columns ex0 - 1 .. ex0 + 3 are all inside the lattice and [ex0, ex0 + 3] is an aligned word
-        const bool interior = ex0 >= 4 && ex0 + 3 <= P.nx - 1;
+    if (ex0 < P.px) {
+        unsigned colset[5] = {0u, 0u, 0u, 0u, 0u};     // bit m: one of the column's four voxels has tag m
+        unsigned tag0[5];                              // tag of (slab 0, row 0, column)
+        unsigned bits[2][5];                           // [row][column]: word of slab 0 (rho, tagged)
+        bool bad = false;
+        // One path for every thread (no divergence at the ends of a row).  Column c is voxel ex0 - 1 + c, clamped to the
+        // lattice.  nx % 4 == 0, so the aligned word [ex0, ex0 + 3] lies inside the row for every ex0 < nx; the last
+        // element column (ex0 == nx: voxels nx - 1 and, clamped, nx - 1 again) takes the row's last word and repeats
+        // its last voxel.  Column 0 is a load of its own at max(ex0 - 1, 0).
+        const int x_left = max(ex0 - 1, 0), x_word = min(ex0, P.nx - 4);
+        const bool past_end = ex0 >= P.nx;
 #pragma unroll
         for (int dz = 0; dz < 2; ++dz) {
             const int iz = min(max(ez + dz - 1, 0), P.nz - 1);
@@ -150,61 +163,53 @@ gdrr_ingest_packed4_kernel(const IngestParams P) {
                 const size_t base = ((size_t)iz * P.ny + iy) * P.nx;
                 unsigned mg[5];
                 float rh[5];
-                if (interior) {
-                    mg[0] = P.mat[base + ex0 - 1];
-                    const unsigned wd = *reinterpret_cast<const unsigned*>(P.mat + base + ex0);
-                    mg[1] = wd & 0xffu; mg[2] = (wd >> 8) & 0xffu; mg[3] = (wd >> 16) & 0xffu; mg[4] = wd >> 24;
-                    if (dz == 0) {
-                        rh[0] = P.rho[base + ex0 - 1];
-                        const float4 f = *reinterpret_cast<const float4*>(P.rho + base + ex0);
-                        rh[1] = f.x; rh[2] = f.y; rh[3] = f.z; rh[4] = f.w;
-                    }
-                } else {
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) {
-                        const int ix = min(max(ex0 - 1 + c, 0), P.nx - 1);      // (element ex's words are voxels ex - 1 and ex)
-                        mg[c] = P.mat[base + ix];
-                        if (dz == 0) rh[c] = P.rho[base + ix];
-                    }
+                mg[0] = P.mat[base + x_left];
+                const unsigned wd = *reinterpret_cast<const unsigned*>(P.mat + base + x_word);
+                mg[4] = wd >> 24;
+                mg[1] = past_end ? mg[4] : (wd & 0xffu);
+                mg[2] = past_end ? mg[4] : ((wd >> 8) & 0xffu);
+                mg[3] = past_end ? mg[4] : ((wd >> 16) & 0xffu);
+                if (dz == 0) {
+                    rh[0] = P.rho[base + x_left];
+                    const float4 f = *reinterpret_cast<const float4*>(P.rho + base + x_word);
+                    rh[4] = f.w;
+                    rh[1] = past_end ? f.w : f.x;
+                    rh[2] = past_end ? f.w : f.y;
+                    rh[3] = past_end ? f.w : f.z;
                 }
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
-                    if ((int)mg[c] >= P.n_mat) *P.bad_flag = 1;
+                    if (dz == 0 && row == 0 && c > 0) bad = bad || (int)mg[c] >= P.n_mat;      // the voxels this thread owns
                     // a voxel whose material belongs to another group of four is an empty voxel (tag 0) of this device volume
-                    const bool here = mg[c] - (unsigned)P.mat_lo < (unsigned)P.n_group;
-                    const unsigned m = here ? mg[c] - (unsigned)P.mat_lo : 0u;
-                    tag[dz][row][c] = m;
+                    const unsigned local = mg[c] - (unsigned)P.mat_lo;
+                    const bool here = local < (unsigned)P.n_group;
+                    const unsigned m = here ? local : 0u;
+                    colset[c] |= 1u << m;
                     if (dz == 0) {
+                        if (row == 0) tag0[c] = m;
                         unsigned b = here ? __float_as_uint(rh[c]) : 0u;
-                        if (P.tagged) b = ((b + 4u) & ~7u) | (m & 3u);
+                        if (P.tagged) b = ((b + 4u) & ~7u) | m;
                         bits[row][c] = b;
                     }
                 }
             }
         }
+        if (bad) *P.bad_flag = 1;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             if (ex0 + e < P.px) {
                 // element ex0 + e: words (x0y0, x0y1, x1y0, x1y1) = columns e, e + 1 of the two rows
                 unsigned w[4] = {bits[0][e], bits[1][e], bits[0][e + 1], bits[1][e + 1]};
-                const unsigned m0 = tag[0][0][e];
-                unsigned mixed = 0u, seen = 0u;
-#pragma unroll
-                for (int dz = 0; dz < 2; ++dz)
-#pragma unroll
-                    for (int row = 0; row < 2; ++row)
-#pragma unroll
-                        for (int dx = 0; dx < 2; ++dx) {
-                            const unsigned m = tag[dz][row][e + dx];
-                            mixed |= m ^ m0;
-                            seen |= 1u << (m & 3u);
-                        }
-                if (P.tagged && mixed == 0u) w[0] |= 4u;
-                if (P.tagged && __popc(seen) == 2) {
-                    const unsigned q = (unsigned)(__ffs((int)(seen & ~(1u << (m0 & 3u)))) - 1);     // the other material
-                    w[1] |= 4u;
-                    w[2] |= (q & 1u) << 2;
-                    w[3] |= (q & 2u) << 1;
+                if (P.tagged) {
+                    const unsigned seen = colset[e] | colset[e + 1];
+                    const int n_seen = __popc(seen);
+                    if (n_seen == 1) w[0] |= 4u;
+                    if (n_seen == 2) {
+                        const unsigned q = (unsigned)(__ffs((int)(seen & ~(1u << tag0[e]))) - 1);     // the other material
+                        w[1] |= 4u;
+                        w[2] |= (q & 1u) << 2;
+                        w[3] |= (q & 2u) << 1;
+                    }
                 }
                 out[e] = make_uint4(w[0], w[1], w[2], w[3]);
             }
@@ -257,8 +262,9 @@ cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_
         // (py and pz, cby and nz stay far below the 65535 limit of grid.y / grid.z for any volume that fits int32 indexing)
         const int row_max = p.sy + 8;                                   // a row, or the last row plus the slab's tail pad
         if (p.nx % 4 == 0 && (uintptr_t)p.mat % 4 == 0 && (uintptr_t)p.rho % 16 == 0) {
-            // four elements per thread, vector loads; 32 threads = 128 elements per block (a C2 row is 257 + pad)
-            gdrr_ingest_packed4_kernel<<<dim3((row_max + 127) / 128, p.py, p.ezn), 32, 0, s>>>(p);
+            // four elements per thread, vector loads; 32 threads = 128 elements of a row per block (a C2 row is 257 + pad)
+            gdrr_ingest_packed4_kernel<<<dim3((row_max + 127) / 128, (p.py + kIngestRows - 1) / kIngestRows, p.ezn),
+                                         dim3(32, kIngestRows), 0, s>>>(p);
             return cudaGetLastError();
         }
         // (64 threads per block: a row of 257 + pad slots, C2, wastes 17% of its threads instead of 48% with 256)
