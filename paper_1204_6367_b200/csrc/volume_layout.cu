@@ -132,7 +132,10 @@ gdrr_ingest_packed_kernel(const IngestParams P) {
 // faces a few more).  A block is 32 threads (x) by kIngestRows rows: neighbouring rows find each other's voxels in L1
 // (measured on C3, ms per ingest: 2 rows 0.341, 4 rows 0.345, 8 rows 0.355; the round's first form of this kernel 0.529).
 // Bit-identical output (tests/test_gpu_ingest.py).
+// GROUPED: the device volume is one of a chain of material groups (mat_lo / n_group map the caller's index to a tag);
+// else tag = material index.
 constexpr int kIngestRows = 2;
+template <bool GROUPED>
 __global__ void __launch_bounds__(32 * kIngestRows)
 gdrr_ingest_packed4_kernel(const IngestParams P) {
     const int ez = P.ez0 + blockIdx.z, ey = kIngestRows * blockIdx.y + threadIdx.y;
@@ -149,9 +152,11 @@ gdrr_ingest_packed4_kernel(const IngestParams P) {
         unsigned bits[2][5];                           // [row][column]: word of slab 0 (rho, tagged)
         bool bad = false;
         // One path for every thread (no divergence at the ends of a row).  Column c is voxel ex0 - 1 + c, clamped to the
-        // lattice.  nx % 4 == 0, so the aligned word [ex0, ex0 + 3] lies inside the row for every ex0 < nx; the last
-        // element column (ex0 == nx: voxels nx - 1 and, clamped, nx - 1 again) takes the row's last word and repeats
-        // its last voxel.  Column 0 is a load of its own at max(ex0 - 1, 0).
+        // lattice.  nx % 4 == 0, so the aligned word [ex0, ex0 + 3] lies inside the row for every ex0 < nx.  The last
+        // element column (ex0 == nx) stores element 0 only, whose columns 0 and 1 are both voxel nx - 1: column 1
+        // repeats column 0 there, and columns 2 .. 4 (the row's last word, so that the load stays in bounds) go unused.
+        // Column 0 is a load of its own at max(ex0 - 1, 0).  (Offsets in int: launch_ingest's caller has checked that
+        // the padded volume fits int32 indexing.)
         const int x_left = max(ex0 - 1, 0), x_word = min(ex0, P.nx - 4);
         const bool past_end = ex0 >= P.nx;
 #pragma unroll
@@ -160,28 +165,26 @@ gdrr_ingest_packed4_kernel(const IngestParams P) {
 #pragma unroll
             for (int row = 0; row < 2; ++row) {
                 const int iy = min(max(ey + row - 1, 0), P.ny - 1);
-                const size_t base = ((size_t)iz * P.ny + iy) * P.nx;
+                const int base = (iz * P.ny + iy) * P.nx;
                 unsigned mg[5];
                 float rh[5];
                 mg[0] = P.mat[base + x_left];
-                const unsigned wd = *reinterpret_cast<const unsigned*>(P.mat + base + x_word);
+                const unsigned wd = *reinterpret_cast<const unsigned*>(P.mat + (base + x_word));
+                mg[1] = past_end ? mg[0] : (wd & 0xffu);
+                mg[2] = (wd >> 8) & 0xffu;
+                mg[3] = (wd >> 16) & 0xffu;
                 mg[4] = wd >> 24;
-                mg[1] = past_end ? mg[4] : (wd & 0xffu);
-                mg[2] = past_end ? mg[4] : ((wd >> 8) & 0xffu);
-                mg[3] = past_end ? mg[4] : ((wd >> 16) & 0xffu);
                 if (dz == 0) {
                     rh[0] = P.rho[base + x_left];
-                    const float4 f = *reinterpret_cast<const float4*>(P.rho + base + x_word);
-                    rh[4] = f.w;
-                    rh[1] = past_end ? f.w : f.x;
-                    rh[2] = past_end ? f.w : f.y;
-                    rh[3] = past_end ? f.w : f.z;
+                    const float4 f = *reinterpret_cast<const float4*>(P.rho + (base + x_word));
+                    rh[1] = past_end ? rh[0] : f.x;
+                    rh[2] = f.y; rh[3] = f.z; rh[4] = f.w;
                 }
 #pragma unroll
                 for (int c = 0; c < 5; ++c) {
                     if (dz == 0 && row == 0 && c > 0) bad = bad || (int)mg[c] >= P.n_mat;      // the voxels this thread owns
                     // a voxel whose material belongs to another group of four is an empty voxel (tag 0) of this device volume
-                    const unsigned local = mg[c] - (unsigned)P.mat_lo;
+                    const unsigned local = GROUPED ? mg[c] - (unsigned)P.mat_lo : mg[c];
                     const bool here = local < (unsigned)P.n_group;
                     const unsigned m = here ? local : 0u;
                     colset[c] |= 1u << m;
@@ -263,8 +266,9 @@ cudaError_t launch_ingest(const IngestParams& p, int vw, int layout, cudaStream_
         const int row_max = p.sy + 8;                                   // a row, or the last row plus the slab's tail pad
         if (p.nx % 4 == 0 && (uintptr_t)p.mat % 4 == 0 && (uintptr_t)p.rho % 16 == 0) {
             // four elements per thread, vector loads; 32 threads = 128 elements of a row per block (a C2 row is 257 + pad)
-            gdrr_ingest_packed4_kernel<<<dim3((row_max + 127) / 128, (p.py + kIngestRows - 1) / kIngestRows, p.ezn),
-                                         dim3(32, kIngestRows), 0, s>>>(p);
+            const dim3 grid((row_max + 127) / 128, (p.py + kIngestRows - 1) / kIngestRows, p.ezn), block(32, kIngestRows);
+            if (p.mat_lo == 0) gdrr_ingest_packed4_kernel<false><<<grid, block, 0, s>>>(p);
+            else gdrr_ingest_packed4_kernel<true><<<grid, block, 0, s>>>(p);
             return cudaGetLastError();
         }
         // (64 threads per block: a row of 257 + pad slots, C2, wastes 17% of its threads instead of 48% with 256)
