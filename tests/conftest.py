@@ -12,6 +12,8 @@ def pytest_addoption(parser):
     parser.addoption("--full-scan", action="store_true", default=False,
                      help="tests/test_gpu_full_scan.py: compare ALL projections of C3 and C4 with the oracle "
                           "(about 25 minutes of oracle time) and write gpurun_out/full_parity_*.json")
+    parser.addoption("--random-cases", action="store", default="0",
+                     help="tests/test_gpu_random_workloads.py: this many further random workloads against the oracle")
 
 
 def pytest_configure(config):

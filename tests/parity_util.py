@@ -22,16 +22,34 @@ def check_signal(sig_gpu, sig_ref, what=""):
 FACE_TIE = 2.0 ** -12       # DESIGN.md reading Q9: a sample this close to a cell face may fall in either cell
 
 
-def face_tie_checker(w, projections):
-    """near_face(index) for check_line_integrals on full images [P][M][nv][nu] of the circular-gantry workload `w`
-    (P = len(projections), indices into w.phis): True iff the oracle's own fp64 positions of that ray have a sample
-    within FACE_TIE of a cell face (reading Q9: the fp32 path may then take the neighbouring cell, whose other
-    corners get a weight <= FACE_TIE)."""
+def oracle_midpoints(w, projection, i, j):
+    """Index coordinates gi[n][3] of every midpoint sample of one ray, from the oracle's own ray record: sample k sits at
+    the parameter (j0 + k + 1/2) step along the unit direction from the source, and gi = (x - centre) / d + (N - 1) / 2
+    (oracle/gdrr_oracle.c index_coords).  Circular gantry or poses; tests/test_parity_util.py pins it to
+    oracle.ray_samples."""
     import oracle
+    if getattr(w, "poses", None) is not None:
+        r = oracle.ray_pose(w, w.poses[projection], i, j)
+    else:
+        r = oracle.ray(w, float(w.phis[projection]), i, j)
+    if not r["hit"] or r["n"] <= 0:
+        return np.zeros((0, 3))
+    t = (r["j0"] + np.arange(r["n"]) + 0.5) * float(w.step_mm)
+    x = r["S"][None, :] + t[:, None] * r["dir"][None, :]
+    d = np.asarray(w.spacing, dtype=np.float64)
+    n = np.asarray(w.dims, dtype=np.float64)
+    return (x - np.asarray(w.centre, dtype=np.float64)[None, :]) / d[None, :] + 0.5 * (n[None, :] - 1.0)
+
+
+def face_tie_checker(w, projections):
+    """near_face(index) for check_line_integrals on full images [P][M][nv][nu] of the workload `w` (P =
+    len(projections), indices into w's projections): True iff the oracle's own fp64 positions of that ray have a
+    sample within FACE_TIE of a cell face (reading Q9: the fp32 path may then take the neighbouring cell, whose other
+    corners get a weight <= FACE_TIE)."""
 
     def near_face(index):
         p, _, j, i = (int(x) for x in index)
-        gi, _ = oracle.ray_samples(w, float(w.phis[projections[p]]), i, j)
+        gi = oracle_midpoints(w, int(projections[p]), i, j)
         if not len(gi):
             return False
         fr = gi - np.floor(gi)
@@ -43,7 +61,7 @@ SLIVER_MM = 1e-3      # two lattice planes of different axes crossed within this
 
 
 def siddon_sliver_checker(w, projections, found=None):
-    """near_face(index) for check_line_integrals on Siddon images [P][M][nv][nu] of the circular-gantry workload `w`:
+    """near_face(index) for check_line_integrals on Siddon images [P][M][nv][nu] of the workload `w` (gantry or poses):
     True iff the ray of that pixel, in the oracle's own fp64 geometry, crosses two lattice planes of DIFFERENT axes
     within SLIVER_MM of path length at a lattice edge one of whose four voxels holds the entry's material with
     rho > 0.  The ray has a sliver of one of those voxels; fp32 can order the two crossings the other way round and
@@ -60,7 +78,10 @@ def siddon_sliver_checker(w, projections, found=None):
         p, m, j, i = (int(x) for x in index)
         if found is not None:
             found.append((int(projections[p]), m, j, i))
-        r = oracle.ray(w, float(w.phis[projections[p]]), i, j)
+        if getattr(w, "poses", None) is not None:
+            r = oracle.ray_pose(w, w.poses[projections[p]], i, j)
+        else:
+            r = oracle.ray(w, float(w.phis[projections[p]]), i, j)
         if not r["hit"]:
             return False
         S, d = r["S"], r["dir"]
@@ -132,7 +153,7 @@ def compare_full(projector, w, oracle_out, what=""):
     sig, li, tab = projector.project(want_li=True, want_table=True)
     sig, li, tab = sig.cpu().numpy(), li.cpu().numpy(), tab.cpu().numpy()
     check_ray_table(tab, oracle_out["ray_table"], what)
-    near_face = face_tie_checker(w, list(range(w.n_proj))) if getattr(w, "poses", None) is None else None
+    near_face = face_tie_checker(w, list(range(w.n_proj)))
     worst_li, n_floor = check_line_integrals(li, oracle_out["line_integrals"], what, near_face)
     worst_sig = check_signal(sig, oracle_out["signal"], what)
     return dict(signal=worst_sig, li=worst_li, li_floor_pixels=n_floor)

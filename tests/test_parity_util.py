@@ -7,7 +7,7 @@ at (u, v) is at y = u s, z = v s where s = (x + 1000) / 1500.
 """
 import numpy as np
 
-from parity_util import face_tie_checker, siddon_sliver_checker
+from parity_util import face_tie_checker, oracle_midpoints, siddon_sliver_checker
 from test_oracle_pins import tiny_workload
 
 
@@ -62,3 +62,27 @@ def test_face_tie_needs_a_midpoint_on_a_cell_face():
     far = tiny_workload(rho, nu=3, nv=3, du=400.0, dv=400.0, phis=[0.0], step=0.5)
     assert not face_tie_checker(far, [0])((0, 0, 0, 0))
     assert not siddon_sliver_checker(far, [0])((0, 0, 0, 0))
+
+
+def test_midpoints_rebuilt_from_the_ray_record_are_the_oracles():
+    """oracle_midpoints (used by the face-tie rule, also for pose workloads) against oracle.ray_samples on the circular
+    gantry, and the pose form against the circular form on the circle's own poses."""
+    import oracle
+    from workloads import trajectories
+    rng = np.random.default_rng(4)
+    rho = rng.uniform(0.0, 2.0, size=(9, 14, 11)).astype(np.float32)
+    phis = np.radians([0.0, 33.0, 147.0, 301.5])
+    w = tiny_workload(rho, spacing=(1.3, 0.9, 2.1), centre=(3.0, -2.0, 1.5), nu=21, nv=17, du=1.4, dv=1.7, phis=phis,
+                      step=0.37, theta=0.004)
+    wp = w.with_poses(trajectories.circular_poses(w.sad, w.sdd, w.theta, phis))
+    seen = 0
+    for p in range(len(phis)):
+        for (i, j) in ((0, 0), (10, 8), (20, 16), (5, 12), (17, 3)):
+            ref, _ = oracle.ray_samples(w, float(phis[p]), i, j)
+            got = oracle_midpoints(w, p, i, j)
+            assert got.shape == ref.shape
+            if len(ref):
+                assert np.abs(got - ref).max() < 1e-12
+                assert np.abs(oracle_midpoints(wp, p, i, j) - ref).max() < 1e-9
+                seen += len(ref)
+    assert seen > 300
