@@ -358,7 +358,7 @@ def run_b200(args):
         rho_h = torch.from_numpy(w.rho).pin_memory()
         mat_h = torch.from_numpy(w.mat).pin_memory()
         out_h = torch.empty((per_gpu, w.nv, w.nu), dtype=torch.float32).pin_memory()
-        stage_proj = min(per_gpu, 32)
+        stage_proj = min(per_gpu, args.e2e_stage)      # the library double-buffers: two batches of stage_proj / 2
         stage = torch.empty((stage_proj, w.nv, w.nu), dtype=torch.float32, device=dev)
 
         def e2e_step():
@@ -546,6 +546,7 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--projections", type=int, default=0, help="projections per GPU (0 = the workload's)")
     ap.add_argument("--launch-proj", type=int, default=0, help="projections per kernel launch (0 = all)")
+    ap.add_argument("--e2e-stage", type=int, default=64, help="projections in the e2e arm's device staging buffer")
     ap.add_argument("--method", default="trilinear", choices=sorted(METHODS) + ["denoise"],
                     help="line integral: the paper's default tri-linear midpoint rule, or its Siddon option")
     ap.add_argument("--sampler", default="auto", choices=["auto", "gather", "staged"],
